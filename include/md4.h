@@ -1,0 +1,144 @@
+/*
+ * md4.h -- C ABI of libmd4: B200-native (sm_100a) FP64 evaluator of 4-center 2-electron repulsion
+ * integrals (ab|cd) over contracted real-solid-harmonic Gaussian shells, matrix form of the
+ * McMurchie-Davidson scheme ("MD4", arXiv:2307.03452).
+ *
+ * Citations: P:n = line n of the paper text, S:8(x) = SURVEY.md section 8(x).
+ *
+ * The engine follows P:200 (section 3): "an engine object is constructed from the given bra and ket
+ * basis sets and the integrals are computed asynchronously for the given bra and ket index pair
+ * lists"; every pair in a list has the same (l_i, l_j) and the same contraction orders (K_i, K_j);
+ * there is no screening: every listed quartet is computed.
+ *
+ * Definition of the result (Eq.1, Eq.6, Eq.16, S:8(c)):
+ *   (ab|cd)_{ma mb mc md} = sum_{ka kb kc kd} c_ka c_kb c_kc c_kd
+ *        Int Int chi^ka_{la ma}(r) chi^kb_{lb mb}(r) |r-r'|^-1 chi^kc_{lc mc}(r') chi^kd_{ld md}(r') d3r d3r'
+ *   chi^k_{lm}(r) = S_lm(r-A) exp(-zeta_k |r-A|^2), S_lm the real solid harmonics in Racah
+ *   normalisation (S_11 = x, S_1-1 = y, S_10 = z, S_20 = z^2 - x^2/2 - y^2/2), m = -l..+l ascending.
+ *   Coefficients are applied verbatim to UNNORMALISED primitives: no hidden normalisation.
+ *
+ * Memory: every pointer argument says HOST or DEVICE.  Host arrays are copied during the call; the
+ * caller may free them on return.  The output buffer is a caller-owned DEVICE buffer.
+ * Errors: every entry point returns md4_status (or writes nothing and returns NULL/void where noted);
+ * nothing throws or aborts across the ABI.  md4_last_error() gives a human-readable reason.
+ * Threading: a context is not thread-safe; distinct contexts are independent.
+ */
+#ifndef MD4_H
+#define MD4_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MD4_LMAX 6 /* highest per-shell angular momentum accepted (i functions) */
+
+typedef struct md4_ctx md4_ctx;     /* opaque engine, one per CUDA device                     */
+typedef struct md4_pairs md4_pairs; /* opaque shell-pair list (device resident), owned by ctx  */
+
+typedef enum {
+    MD4_OK = 0,
+    MD4_EINVAL = 1,       /* bad argument: null pointer, index out of range, class mix, zeta <= 0 */
+    MD4_EUNSUPPORTED = 2, /* l > MD4_LMAX                                                          */
+    MD4_ESTATE = 3,       /* call order: pairs before shells, pairs of another context             */
+    MD4_ENOMEM = 4,       /* host or device allocation failed                                      */
+    MD4_ECUDA = 5         /* CUDA runtime error; text in md4_last_error                            */
+} md4_status;
+
+/* Create an engine on CUDA device `cuda_device`.  Builds the constant device tables: Hermite
+ * ordinals and the R-recurrence table (Listing 3.1), Cartesian->solid-harmonic coefficients
+ * (Eq.16) and the Boys interpolation table (Eq.11).  *out is NULL on failure. */
+md4_status md4_create(md4_ctx** out, int cuda_device);
+
+/* Free the engine, its shells, every pair list still alive and all workspaces.  NULL is a no-op. */
+void md4_destroy(md4_ctx* ctx);
+
+/* Text of the last failure on this context (ctx-owned, valid until the next call on ctx; never freed
+ * by the caller).  With ctx == NULL returns the text of the last failed md4_create on this thread. */
+const char* md4_last_error(const md4_ctx* ctx);
+
+/* Upload shells exactly as the paper states the problem (Eq.1): centre, l, primitive
+ * exponents, contraction coefficients.  Replaces any previous shell set; existing pair lists stay
+ * valid (they hold their own data).
+ *   centers_xyz   HOST [nshell*3]  bohr
+ *   l             HOST [nshell]    0..MD4_LMAX
+ *   prim_offset   HOST [nshell+1]  CSR offsets into exponents/coefficients, prim_offset[0] = 0, increasing
+ *   exponents     HOST [nprim]     > 0, finite
+ *   coefficients  HOST [nprim]     finite, applied verbatim
+ * nshell == 0 is accepted (clears the shell set). */
+md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, const int* l,
+                          const int* prim_offset, const double* exponents, const double* coefficients);
+
+/* Shell-pair precompute (S:8(a) a1; Eq.3-5, Eq.16, Listing 2.1 lines 2-3):
+ * for every listed ordered pair (i,j) and every primitive pair (ka,kb) computes zeta_p, R_p,
+ * ln K_ab = -zeta_a zeta_b/zeta_p |AB|^2 and the matrix H (solid-harmonic pair index x Hermite index)
+ * = c_ka c_kb * C_la (x) C_lb * E, on the device.  All pairs must share (l_i, l_j, K_i, K_j), else
+ * MD4_EINVAL.  A list is role-agnostic: the same list may serve as bra and as ket.
+ *   ij   HOST [npair*2]  shell indices (i0,j0,i1,j1,...)
+ * npair == 0 gives a valid empty list.  *out is NULL on failure. */
+md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** out);
+
+/* Release one pair list (also done by md4_destroy).  NULL is a no-op. */
+void md4_free_pairs(md4_ctx* ctx, md4_pairs* pairs);
+
+/* Shape queries of a pair list; return -1 for NULL. */
+int md4_pairs_count(const md4_pairs* pairs);
+/* info[0..3] = l_i, l_j, K_i, K_j (HOST [4]). */
+md4_status md4_pairs_class(const md4_pairs* pairs, int* info);
+
+/* Number of doubles md4_compute writes: npair_bra * npair_ket * (2la+1)(2lb+1)(2lc+1)(2ld+1). */
+md4_status md4_output_size(const md4_pairs* bra, const md4_pairs* ket, size_t* n_doubles);
+
+/* Compute every quartet of (bra list) x (ket list) (S:8(a) a2-a9; Eq.6-15, P:115-128 Listing
+ * 2.1): Boys F_m(T) -> Hermite Coulomb tensor R by the recurrence Eq.13 in shared memory -> bra
+ * transform [ab|q~] = sum_p~ H_ab [p~|q~] -> ket transform (ab|cd) = sum_q~ [ab|q~] H_cd, accumulated
+ * over primitive quartets, FP64 throughout.
+ *   d_out   DEVICE, 8-byte aligned, capacity_doubles >= md4_output_size; fully OVERWRITTEN with
+ *           out[i_bra][j_ket][ma][mb][mc][md], row-major, md fastest, m = -l..+l ascending.
+ *   cuda_stream  the caller's cudaStream_t (NULL = default stream).  The call only enqueues work on
+ *           that stream and returns: no device synchronisation, no allocation.
+ * On any error nothing is enqueued.  Empty lists: MD4_OK, nothing written. */
+md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out,
+                       size_t capacity_doubles, void* cuda_stream);
+
+/* Same through HOST buffers (the end-to-end path bench.py's "e2e" times): copies the result to
+ * h_out [capacity_doubles] (HOST) through an internal device buffer that grows on demand, and
+ * synchronises the stream before returning. */
+md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* h_out,
+                            size_t capacity_doubles, void* cuda_stream);
+
+/* Number of kernel launches this context has enqueued so far (bench.py's "gpu_launches"). */
+long long md4_launch_count(const md4_ctx* ctx);
+
+/* Algorithmic FLOPs per shell quartet for bra x ket, matrix operations only, bra transformed first
+ * (Eq.17-18): Kbra Kket 2 Nab Np Nq + Kket 2 Nab Nq Ncd.  0 for NULL. */
+double md4_flops_per_quartet(const md4_pairs* bra, const md4_pairs* ket);
+
+/* ---- stage-level access for the parity tests (S:4 test layer 3) --------------------------------- */
+
+/* Boys function F_m(T), m = 0..mmax (mmax <= 4*MD4_LMAX), evaluated on the device by the same device
+ * function the compute kernel uses (table + Taylor, asymptotic above T_max).
+ *   T HOST [n], out HOST [n*(mmax+1)] */
+md4_status md4_debug_boys(md4_ctx* ctx, int mmax, int n, const double* T, double* out);
+
+/* Cartesian->solid coefficient table of the library for one l: out HOST [(2l+1) * (l+1)(l+2)/2],
+ * row m+l, Cartesian triples ordered x descending then y descending. */
+md4_status md4_debug_solid_coeff(md4_ctx* ctx, int l, double* out);
+
+/* Hermite Coulomb tensor R^{(0)}_{tuv}, t+u+v <= L (L <= 4*MD4_LMAX), for one primitive quartet given
+ * by (zeta_p, P, zeta_q, Q); prefactor 2 pi^{5/2}/(zeta_p zeta_q sqrt(zeta_p+zeta_q)) included, no K_ab.
+ * pq HOST [8] = zeta_p, Px, Py, Pz, zeta_q, Qx, Qy, Qz; out HOST [(L+1)^3] indexed t*(L+1)^2+u*(L+1)+v
+ * (entries with t+u+v > L are set to 0). */
+md4_status md4_debug_hermite_r(md4_ctx* ctx, int L, const double* pq, double* out);
+
+/* H matrix of primitive pair `iprim` (ka*Kj+kb) of pair `ipair`: out HOST [Nab * Np] row-major,
+ * Nab = (2li+1)(2lj+1), Np = (lbra+1)(lbra+2)(lbra+3)/6, Hermite index ordered by degree t+u+v, then t
+ * descending, then u descending; also scal HOST [5] = zeta_p, Px, Py, Pz, ln K_ab. */
+md4_status md4_debug_pair_h(md4_ctx* ctx, const md4_pairs* pairs, int ipair, int iprim, double* out,
+                            double* scal);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD4_H */

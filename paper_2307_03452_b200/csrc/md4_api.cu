@@ -1,0 +1,336 @@
+// md4_api.cu -- the C ABI of include/md4.h: context, shells, pair lists, compute dispatch.
+// Host logic only; every step of the hot path runs in the kernels of md4_pairs.cu / md4_eri.cu.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "md4_internal.h"
+
+using namespace md4;
+
+namespace {
+thread_local std::string g_create_err;
+
+template <class T>
+cudaError_t upload(std::vector<void*>* keep, const T* h, size_t n, T** d) {
+    *d = nullptr;
+    cudaError_t e = cudaMalloc((void**)d, (n ? n : 1) * sizeof(T));
+    if (e != cudaSuccess) return e;
+    if (keep) keep->push_back(*d);
+    if (n) e = cudaMemcpy(*d, h, n * sizeof(T), cudaMemcpyHostToDevice);
+    return e;
+}
+
+md4_status fail(md4_ctx* ctx, md4_status s, const std::string& msg) {
+    if (ctx) ctx->err = msg;
+    return s;
+}
+md4_status cuda_fail(md4_ctx* ctx, const char* what, cudaError_t e) {
+    (void)cudaGetLastError();
+    return fail(ctx, e == cudaErrorMemoryAllocation ? MD4_ENOMEM : MD4_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+void free_shells(md4_ctx* c) {
+    cudaFree(c->d_centers); cudaFree(c->d_l); cudaFree(c->d_off); cudaFree(c->d_exp); cudaFree(c->d_coef);
+    c->d_centers = nullptr; c->d_l = nullptr; c->d_off = nullptr; c->d_exp = nullptr; c->d_coef = nullptr;
+    c->nshell = 0; c->nprim = 0; c->h_l.clear(); c->h_off.clear();
+}
+
+void free_pair_storage(md4_pairs* p) {
+    cudaFree(p->d.H); cudaFree(p->d.scal); cudaFree(p->d.pairmax); cudaFree(p->d.ij);
+    delete p;
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok;
+    explicit DeviceGuard(int dev) {
+        ok = cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+}  // namespace
+
+extern "C" {
+
+md4_status md4_create(md4_ctx** out, int cuda_device) {
+    if (!out) { g_create_err = "md4_create: out is NULL"; return MD4_EINVAL; }
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); g_create_err = std::string("md4_create: no CUDA device: ") + cudaGetErrorString(e); return MD4_ECUDA; }
+    if (cuda_device < 0 || cuda_device >= ndev) { g_create_err = "md4_create: cuda_device out of range"; return MD4_EINVAL; }
+    md4_ctx* c = new (std::nothrow) md4_ctx();
+    if (!c) { g_create_err = "md4_create: out of host memory"; return MD4_ENOMEM; }
+    c->device = cuda_device;
+    DeviceGuard g(cuda_device);
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, cuda_device);
+    if (e != cudaSuccess) { g_create_err = std::string("md4_create: ") + cudaGetErrorString(e); delete c; return MD4_ECUDA; }
+    if (prop.major < 10) { g_create_err = "md4_create: libmd4 is built for sm_100a (B200) only"; delete c; return MD4_EUNSUPPORTED; }
+    c->num_sms = prop.multiProcessorCount;
+    c->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    build_host_tables(c->htab);
+    uint32_t *d_rtab = nullptr, *d_tuv = nullptr;
+    double* d_boys = nullptr;
+    e = upload(&c->table_allocs, c->htab.rtab.data(), c->htab.rtab.size(), &d_rtab);
+    if (e == cudaSuccess) e = upload(&c->table_allocs, c->htab.tuv.data(), c->htab.tuv.size(), &d_tuv);
+    if (e == cudaSuccess) e = upload(&c->table_allocs, c->htab.boys.data(), c->htab.boys.size(), &d_boys);
+    c->tab.rtab = d_rtab; c->tab.tuv = d_tuv; c->tab.boys = d_boys;
+    for (int l = 0; l <= LMAX && e == cudaSuccess; ++l) {
+        double* d = nullptr;
+        e = upload(&c->table_allocs, c->htab.solid[l].data(), c->htab.solid[l].size(), &d);
+        c->tab.solid[l] = d;
+    }
+    if (e != cudaSuccess) {
+        g_create_err = std::string("md4_create: table upload: ") + cudaGetErrorString(e);
+        for (void* p : c->table_allocs) cudaFree(p);
+        delete c;
+        return e == cudaErrorMemoryAllocation ? MD4_ENOMEM : MD4_ECUDA;
+    }
+    *out = c;
+    return MD4_OK;
+}
+
+void md4_destroy(md4_ctx* ctx) {
+    if (!ctx) return;
+    DeviceGuard g(ctx->device);
+    for (md4_pairs* p : ctx->lists) free_pair_storage(p);
+    ctx->lists.clear();
+    free_shells(ctx);
+    cudaFree(ctx->d_scratch);
+    for (void* p : ctx->table_allocs) cudaFree(p);
+    delete ctx;
+}
+
+const char* md4_last_error(const md4_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, const int* l, const int* prim_offset,
+                          const double* exponents, const double* coefficients) {
+    if (!ctx) return MD4_EINVAL;
+    if (nshell < 0) return fail(ctx, MD4_EINVAL, "md4_set_shells: nshell < 0");
+    if (nshell > 0 && (!centers_xyz || !l || !prim_offset || !exponents || !coefficients))
+        return fail(ctx, MD4_EINVAL, "md4_set_shells: null array");
+    int nprim = 0;
+    if (nshell > 0) {
+        if (prim_offset[0] != 0) return fail(ctx, MD4_EINVAL, "md4_set_shells: prim_offset[0] != 0");
+        for (int i = 0; i < nshell; ++i) {
+            if (l[i] < 0) return fail(ctx, MD4_EINVAL, "md4_set_shells: l < 0");
+            if (l[i] > LMAX) return fail(ctx, MD4_EUNSUPPORTED, "md4_set_shells: l > MD4_LMAX");
+            if (prim_offset[i + 1] <= prim_offset[i]) return fail(ctx, MD4_EINVAL, "md4_set_shells: shell without primitives");
+            for (int k = 0; k < 3; ++k)
+                if (!std::isfinite(centers_xyz[3 * i + k])) return fail(ctx, MD4_EINVAL, "md4_set_shells: centre not finite");
+        }
+        nprim = prim_offset[nshell];
+        for (int k = 0; k < nprim; ++k) {
+            if (!(exponents[k] > 0.0) || !std::isfinite(exponents[k])) return fail(ctx, MD4_EINVAL, "md4_set_shells: exponent must be > 0 and finite");
+            if (!std::isfinite(coefficients[k])) return fail(ctx, MD4_EINVAL, "md4_set_shells: coefficient not finite");
+        }
+    }
+    DeviceGuard g(ctx->device);
+    free_shells(ctx);
+    if (nshell == 0) return MD4_OK;
+    cudaError_t e = upload<double>(nullptr, centers_xyz, (size_t)nshell * 3, &ctx->d_centers);
+    if (e == cudaSuccess) e = upload<int>(nullptr, l, nshell, &ctx->d_l);
+    if (e == cudaSuccess) e = upload<int>(nullptr, prim_offset, (size_t)nshell + 1, &ctx->d_off);
+    if (e == cudaSuccess) e = upload<double>(nullptr, exponents, nprim, &ctx->d_exp);
+    if (e == cudaSuccess) e = upload<double>(nullptr, coefficients, nprim, &ctx->d_coef);
+    if (e != cudaSuccess) { free_shells(ctx); return cuda_fail(ctx, "md4_set_shells", e); }
+    ctx->nshell = nshell; ctx->nprim = nprim;
+    ctx->h_l.assign(l, l + nshell);
+    ctx->h_off.assign(prim_offset, prim_offset + nshell + 1);
+    return MD4_OK;
+}
+
+md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** out) {
+    if (!ctx) return MD4_EINVAL;
+    if (!out) return fail(ctx, MD4_EINVAL, "md4_build_pairs: out is NULL");
+    *out = nullptr;
+    if (npair < 0) return fail(ctx, MD4_EINVAL, "md4_build_pairs: npair < 0");
+    if (npair > 0 && !ij) return fail(ctx, MD4_EINVAL, "md4_build_pairs: ij is NULL");
+    if (npair > 0 && ctx->nshell == 0) return fail(ctx, MD4_ESTATE, "md4_build_pairs: no shells uploaded");
+    PairListDev d;
+    std::memset(&d, 0, sizeof(d));
+    d.npair = npair;
+    d.Ki = d.Kj = 1;
+    for (int p = 0; p < npair; ++p) {
+        const int i = ij[2 * p], j = ij[2 * p + 1];
+        if (i < 0 || j < 0 || i >= ctx->nshell || j >= ctx->nshell) return fail(ctx, MD4_EINVAL, "md4_build_pairs: shell index out of range");
+        const int li = ctx->h_l[i], lj = ctx->h_l[j];
+        const int Ki = ctx->h_off[i + 1] - ctx->h_off[i], Kj = ctx->h_off[j + 1] - ctx->h_off[j];
+        if (p == 0) { d.li = li; d.lj = lj; d.Ki = Ki; d.Kj = Kj; }
+        else if (li != d.li || lj != d.lj || Ki != d.Ki || Kj != d.Kj)
+            return fail(ctx, MD4_EINVAL, "md4_build_pairs: pairs of one list must share (l_i, l_j, K_i, K_j) (P:200)");
+    }
+    d.lsum = d.li + d.lj;
+    d.nab = n_solid(d.li) * n_solid(d.lj);
+    d.nrb = (d.nab + 7) / 8;
+    d.nherm = n_hermite(d.lsum);
+    d.ncb = (d.nherm + 7) / 8;
+    d.hstride = (size_t)d.ncb * d.nrb * 64;
+    md4_pairs* pl = new (std::nothrow) md4_pairs();
+    if (!pl) return fail(ctx, MD4_ENOMEM, "md4_build_pairs: out of host memory");
+    pl->ctx = ctx;
+    pl->d = d;
+    if (npair > 0) {
+        DeviceGuard g(ctx->device);
+        const size_t nprim = (size_t)npair * d.Ki * d.Kj;
+        cudaError_t e = cudaMalloc((void**)&pl->d.H, nprim * d.hstride * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.scal, nprim * 8 * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.pairmax, (size_t)npair * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.ij, (size_t)npair * 2 * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemcpy(pl->d.ij, ij, (size_t)npair * 2 * sizeof(int), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = launch_pair_kernel(ctx, pl->d, 0);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+        if (e != cudaSuccess) { free_pair_storage(pl); return cuda_fail(ctx, "md4_build_pairs", e); }
+    }
+    ctx->lists.insert(pl);
+    *out = pl;
+    return MD4_OK;
+}
+
+void md4_free_pairs(md4_ctx* ctx, md4_pairs* pairs) {
+    if (!ctx || !pairs) return;
+    auto it = ctx->lists.find(pairs);
+    if (it == ctx->lists.end()) return;
+    ctx->lists.erase(it);
+    DeviceGuard g(ctx->device);
+    free_pair_storage(pairs);
+}
+
+int md4_pairs_count(const md4_pairs* pairs) { return pairs ? pairs->d.npair : -1; }
+
+md4_status md4_pairs_class(const md4_pairs* pairs, int* info) {
+    if (!pairs || !info) return MD4_EINVAL;
+    info[0] = pairs->d.li; info[1] = pairs->d.lj; info[2] = pairs->d.Ki; info[3] = pairs->d.Kj;
+    return MD4_OK;
+}
+
+md4_status md4_output_size(const md4_pairs* bra, const md4_pairs* ket, size_t* n_doubles) {
+    if (!bra || !ket || !n_doubles) return MD4_EINVAL;
+    *n_doubles = (size_t)bra->d.npair * ket->d.npair * bra->d.nab * ket->d.nab;
+    return MD4_OK;
+}
+
+double md4_flops_per_quartet(const md4_pairs* bra, const md4_pairs* ket) {
+    if (!bra || !ket) return 0.0;
+    const double kb = (double)bra->d.Ki * bra->d.Kj, kk = (double)ket->d.Ki * ket->d.Kj;
+    return kb * kk * 2.0 * bra->d.nab * bra->d.nherm * ket->d.nherm + kk * 2.0 * bra->d.nab * ket->d.nherm * ket->d.nab;
+}
+
+long long md4_launch_count(const md4_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+static md4_status check_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, const void* out, size_t cap,
+                                size_t* need) {
+    if (!ctx) return MD4_EINVAL;
+    if (!bra || !ket) return fail(ctx, MD4_EINVAL, "md4_compute: pair list is NULL");
+    if (bra->ctx != ctx || ket->ctx != ctx || !ctx->lists.count(const_cast<md4_pairs*>(bra)) ||
+        !ctx->lists.count(const_cast<md4_pairs*>(ket)))
+        return fail(ctx, MD4_ESTATE, "md4_compute: pair list does not belong to this context");
+    md4_output_size(bra, ket, need);
+    if (*need == 0) return MD4_OK;
+    if (!out) return fail(ctx, MD4_EINVAL, "md4_compute: output pointer is NULL");
+    if (((uintptr_t)out & 7) != 0) return fail(ctx, MD4_EINVAL, "md4_compute: output pointer not 8-byte aligned");
+    if (cap < *need) return fail(ctx, MD4_EINVAL, "md4_compute: output capacity too small");
+    return MD4_OK;
+}
+
+md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out, size_t capacity_doubles,
+                       void* cuda_stream) {
+    size_t need = 0;
+    md4_status s = check_compute(ctx, bra, ket, d_out, capacity_doubles, &need);
+    if (s != MD4_OK || need == 0) return s;
+    DeviceGuard g(ctx->device);
+    return launch_eri(ctx, bra->d, ket->d, d_out, (cudaStream_t)cuda_stream);
+}
+
+md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* h_out,
+                            size_t capacity_doubles, void* cuda_stream) {
+    size_t need = 0;
+    md4_status s = check_compute(ctx, bra, ket, h_out, capacity_doubles, &need);
+    if (s != MD4_OK || need == 0) return s;
+    DeviceGuard g(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (ctx->scratch_doubles < need) {
+        cudaFree(ctx->d_scratch);
+        ctx->d_scratch = nullptr; ctx->scratch_doubles = 0;
+        cudaError_t e = cudaMalloc((void**)&ctx->d_scratch, need * sizeof(double));
+        if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
+        ctx->scratch_doubles = need;
+    }
+    s = launch_eri(ctx, bra->d, ket->d, ctx->d_scratch, st);
+    if (s != MD4_OK) return s;
+    cudaError_t e = cudaMemcpyAsync(h_out, ctx->d_scratch, need * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
+    return MD4_OK;
+}
+
+md4_status md4_debug_boys(md4_ctx* ctx, int mmax, int n, const double* T, double* out) {
+    if (!ctx) return MD4_EINVAL;
+    if (mmax < 0 || mmax > LTOT || n < 0 || (n > 0 && (!T || !out))) return fail(ctx, MD4_EINVAL, "md4_debug_boys: bad argument");
+    if (n == 0) return MD4_OK;
+    for (int i = 0; i < n; ++i)
+        if (!(T[i] >= 0.0) || !std::isfinite(T[i])) return fail(ctx, MD4_EINVAL, "md4_debug_boys: T must be >= 0 and finite");
+    DeviceGuard g(ctx->device);
+    double *dT = nullptr, *dO = nullptr;
+    const size_t no = (size_t)n * (mmax + 1);
+    cudaError_t e = cudaMalloc((void**)&dT, n * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&dO, no * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(dT, T, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_debug_boys(ctx, mmax, n, dT, dO);
+    if (e == cudaSuccess) e = cudaMemcpy(out, dO, no * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(dT); cudaFree(dO);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_debug_boys", e);
+    return MD4_OK;
+}
+
+md4_status md4_debug_solid_coeff(md4_ctx* ctx, int l, double* out) {
+    if (!ctx) return MD4_EINVAL;
+    if (l < 0 || l > LMAX || !out) return fail(ctx, MD4_EINVAL, "md4_debug_solid_coeff: bad argument");
+    DeviceGuard g(ctx->device);
+    cudaError_t e = cudaMemcpy(out, ctx->tab.solid[l], (size_t)n_solid(l) * n_cart(l) * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_debug_solid_coeff", e);
+    return MD4_OK;
+}
+
+md4_status md4_debug_hermite_r(md4_ctx* ctx, int L, const double* pq, double* out) {
+    if (!ctx) return MD4_EINVAL;
+    if (L < 0 || L > LTOT || !pq || !out) return fail(ctx, MD4_EINVAL, "md4_debug_hermite_r: bad argument");
+    if (!(pq[0] > 0.0) || !(pq[4] > 0.0)) return fail(ctx, MD4_EINVAL, "md4_debug_hermite_r: exponents must be > 0");
+    DeviceGuard g(ctx->device);
+    const size_t no = (size_t)(L + 1) * (L + 1) * (L + 1);
+    double *dP = nullptr, *dO = nullptr;
+    cudaError_t e = cudaMalloc((void**)&dP, 8 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&dO, no * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(dP, pq, 8 * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_debug_r(ctx, L, dP, dO);
+    if (e == cudaSuccess) e = cudaMemcpy(out, dO, no * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(dP); cudaFree(dO);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_debug_hermite_r", e);
+    return MD4_OK;
+}
+
+md4_status md4_debug_pair_h(md4_ctx* ctx, const md4_pairs* pairs, int ipair, int iprim, double* out, double* scal) {
+    if (!ctx) return MD4_EINVAL;
+    if (!pairs || !out || !scal) return fail(ctx, MD4_EINVAL, "md4_debug_pair_h: null argument");
+    if (!ctx->lists.count(const_cast<md4_pairs*>(pairs))) return fail(ctx, MD4_ESTATE, "md4_debug_pair_h: foreign pair list");
+    const PairListDev& d = pairs->d;
+    const int kk = d.Ki * d.Kj;
+    if (ipair < 0 || ipair >= d.npair || iprim < 0 || iprim >= kk) return fail(ctx, MD4_EINVAL, "md4_debug_pair_h: index out of range");
+    DeviceGuard g(ctx->device);
+    std::vector<double> blk(d.hstride);
+    double s8[8], pm = 0.0;
+    const size_t ip = (size_t)ipair * kk + iprim;
+    cudaError_t e = cudaMemcpy(blk.data(), d.H + ip * d.hstride, d.hstride * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(s8, d.scal + ip * 8, sizeof(s8), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(&pm, d.pairmax + ipair, sizeof(double), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_debug_pair_h", e);
+    for (int r = 0; r < d.nab; ++r)
+        for (int c = 0; c < d.nherm; ++c)
+            out[(size_t)r * d.nherm + c] = blk[((size_t)(c >> 3) * d.nrb + (r >> 3)) * 64 + (r & 7) * 8 + (c & 7)];
+    scal[0] = s8[0]; scal[1] = s8[1]; scal[2] = s8[2]; scal[3] = s8[3]; scal[4] = s8[4] + pm;
+    return MD4_OK;
+}
+
+}  // extern "C"

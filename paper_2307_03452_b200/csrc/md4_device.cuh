@@ -1,0 +1,101 @@
+// md4_device.cuh -- device functions shared by the compute kernel and the stage-level debug kernels:
+// Boys function (Eq.11), seeds [0]^(m) (Eq.10, Eq.12) and the Hermite Coulomb tensor
+// recurrence Eq.13 level by level in shared memory (after Listing 3.1).
+#pragma once
+#include "md4_internal.h"
+
+namespace md4 {
+
+// F_m(T): table of F_{m..m+7}(T_j) at the nearest node T_j = j/16 and a 7th-order Taylor step
+// F_m(T) = sum_k F_{m+k}(T_j) (T_j - T)^k / k!  (remainder <= (1/32)^8/8! = 2.3e-17 relative);
+// T >= 100: F_m = (2m-1)!!/(2T)^m sqrt(pi/T)/2 (relative error < 1e-19 for m <= 24; S:8(c) Q11).
+__device__ __forceinline__ double boys_one(const double* __restrict__ tab, int m, double T) {
+    if (T < (double)BOYS_TMAX) {
+        const int j = (int)(T * BOYS_INV_DELTA + 0.5);
+        const double d = (double)j * (1.0 / BOYS_INV_DELTA) - T;
+        const double* f = tab + (size_t)j * BOYS_STRIDE + m;
+        double r = __ldg(f + 7) * (1.0 / 5040.0);
+        r = fma(r, d, __ldg(f + 6) * (1.0 / 720.0));
+        r = fma(r, d, __ldg(f + 5) * (1.0 / 120.0));
+        r = fma(r, d, __ldg(f + 4) * (1.0 / 24.0));
+        r = fma(r, d, __ldg(f + 3) * (1.0 / 6.0));
+        r = fma(r, d, __ldg(f + 2) * 0.5);
+        r = fma(r, d, __ldg(f + 1));
+        r = fma(r, d, __ldg(f));
+        return r;
+    }
+    const double inv = 0.5 / T;
+    double r = 0.5 * sqrt(3.14159265358979323846 / T);
+    for (int k = 0; k < m; ++k) r *= (2 * k + 1) * inv;
+    return r;
+}
+
+// Builds R^{(0)}_{tuv}, t+u+v <= L, for one primitive quartet into Ra[t*S*S + u*S + v] (S = L+1).
+// All threads of the CTA must call it.  Rc0/Rc1: two scratch arrays of n_hermite(L) doubles, sS: 32 doubles.
+// scale multiplies every value (K_ab K_cd relative to the pair maxima; 1 in the debug kernel).
+// Level l = 1..L computes [r]^(L-l) for all |r| <= l from level l-1 (one barrier per level, ping-pong
+// buffers instead of the paper's in-place array with two barriers; the last level scatters into the
+// additive layout so that address(p~ + q~) = address(p~) + address(q~), Eq.8 as a pure gather).
+__device__ __forceinline__ void hermite_r_block(double* Ra, double* Rc0, double* Rc1, double* sS,
+                                                const uint32_t* __restrict__ rtab,
+                                                const uint32_t* __restrict__ tuv,
+                                                const double* __restrict__ boys, int L, int S, double zp,
+                                                double Px, double Py, double Pz, double zq, double Qx, double Qy,
+                                                double Qz, double scale, int tid, int nthr) {
+    const double X0 = Px - Qx, X1 = Py - Qy, X2 = Pz - Qz;
+    if (tid < 32) {
+        const double zs = zp + zq;
+        const double rho = zp * zq / zs;
+        const double T = rho * (X0 * X0 + X1 * X1 + X2 * X2);
+        // 2 pi^{5/2} = 34.98683665524972497
+        const double pref = scale * 34.986836655249724970 / (zp * zq * sqrt(zs));
+        if (tid <= L) {
+            const double F = boys_one(boys, tid, T);
+            double pw = pref;
+            const double m2r = -2.0 * rho;
+            for (int k = 0; k < tid; ++k) pw *= m2r;
+            sS[tid] = pw * F;
+        }
+    }
+    __syncthreads();
+    if (L == 0) {
+        if (tid == 0) Ra[0] = sS[0];
+        __syncthreads();
+        return;
+    }
+    double* src = Rc0;
+    double* dst = Rc1;
+    if (tid == 0) src[0] = sS[L];
+    __syncthreads();
+    for (int l = 1; l <= L; ++l) {
+        const int n = n_hermite(l);
+        const bool last = (l == L);
+        for (int e = tid; e < n; e += nthr) {
+            double val;
+            if (e == 0) {
+                val = sS[L - l];
+            } else {
+                const uint32_t w = __ldg(rtab + e);
+                const int i0 = w & 4095, i1 = (w >> 12) & 4095, C = (w >> 24) & 31, ax = (w >> 29) & 3;
+                const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
+                val = fma((double)C, src[i0], x * src[i1]);
+            }
+            if (last) {
+                const uint32_t q = __ldg(tuv + e);
+                Ra[((q & 255) * S + ((q >> 8) & 255)) * S + ((q >> 16) & 255)] = val;
+            } else {
+                dst[e] = val;
+            }
+        }
+        __syncthreads();
+        double* t = src; src = dst; dst = t;
+    }
+}
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+}  // namespace md4

@@ -1,0 +1,104 @@
+// md4_internal.h -- declarations shared by the translation units of libmd4 (never by the oracle).
+// Citations: P:n = PAPER.md line n, S:8(x) = SURVEY.md section 8(x).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include <set>
+
+#include "../../include/md4.h"
+
+namespace md4 {
+
+constexpr int LMAX = MD4_LMAX;          // per shell
+constexpr int LTOT = 4 * LMAX;          // highest Hermite order L = la+lb+lc+ld
+constexpr int NR_MAX = (LTOT + 1) * (LTOT + 2) * (LTOT + 3) / 6;  // 2925
+
+// Boys table: nodes T_j = j / BOYS_INV_DELTA, j = 0..BOYS_NODES-1, values F_m(T_j) for m = 0..BOYS_STRIDE-1.
+constexpr int BOYS_INV_DELTA = 16;
+constexpr int BOYS_TMAX = 100;          // above: asymptotic form (relative error < 1e-19 for m <= 24, S:8(c) Q11)
+constexpr int BOYS_NODES = BOYS_TMAX * BOYS_INV_DELTA + 1;
+constexpr int BOYS_TAYLOR = 8;          // terms k = 0..7
+constexpr int BOYS_STRIDE = LTOT + BOYS_TAYLOR;  // 32
+
+__host__ __device__ inline int n_hermite(int n) { return (n + 1) * (n + 2) * (n + 3) / 6; }
+__host__ __device__ inline int n_cart(int l) { return (l + 1) * (l + 2) / 2; }
+__host__ __device__ inline int n_solid(int l) { return 2 * l + 1; }
+
+// Graded Hermite ordinal (all |r| <= n first, needed by the in-place-style level recurrence):
+// degree ascending, then t descending, then u descending.
+__host__ __device__ inline int herm_ord(int t, int u, int v) {
+    int n = t + u + v;
+    int w = n - t;
+    return n * (n + 1) * (n + 2) / 6 + w * (w + 1) / 2 + (w - u);
+}
+
+// Constant device tables, built once per context (md4_tables.cpp).
+struct DeviceTables {
+    const uint32_t* rtab;    // [NR_MAX] packed {idx0:12, idx1:12, C:5, axis:2} of Eq.13
+    const uint32_t* tuv;     // [NR_MAX] packed t | u << 8 | v << 16 in graded order
+    const double* boys;      // [BOYS_NODES * BOYS_STRIDE]
+    const double* solid[LMAX + 1];  // [(2l+1) * n_cart(l)]
+};
+
+struct HostTables {
+    std::vector<uint32_t> rtab, tuv;
+    std::vector<double> boys;
+    std::vector<double> solid[LMAX + 1];
+};
+void build_host_tables(HostTables& t);  // md4_tables.cpp
+
+// H matrices are stored in 8x8 blocks: element (row, col) of primitive pair ip lives at
+//   H[ip * hstride + ((col/8) * nrb + row/8) * 64 + (row%8) * 8 + col%8],
+// rows = solid-harmonic pair index ma*(2lj+1)+mb padded to nrb*8, cols = Hermite ordinal padded to
+// ncb*8, padding = 0.  One block is exactly the A fragment pair (bra role) or the B fragment pair
+// (ket role) of two DMMA.8x8x4 k-steps for a warp (lane*2 + {0,1}).
+struct PairListDev {
+    int npair, li, lj, Ki, Kj;
+    int lsum, nab, nrb, nherm, ncb;
+    size_t hstride;      // doubles per primitive pair
+    double* H;           // [npair*Ki*Kj * hstride]
+    double* scal;        // [npair*Ki*Kj * 8]: zeta_p, Px, Py, Pz, lnK - pairmax, 0, 0, 0
+    double* pairmax;     // [npair] max over primitives of ln K_ab
+    int* ij;             // [npair*2]
+};
+
+}  // namespace md4
+
+struct md4_pairs {
+    md4_ctx* ctx;
+    md4::PairListDev d;
+};
+
+struct md4_ctx {
+    int device;
+    std::string err;
+    md4::DeviceTables tab;
+    std::vector<void*> table_allocs;
+    // shells (device)
+    int nshell = 0, nprim = 0;
+    double* d_centers = nullptr;
+    int* d_l = nullptr;
+    int* d_off = nullptr;
+    double* d_exp = nullptr;
+    double* d_coef = nullptr;
+    std::vector<int> h_l, h_off;
+    std::set<md4_pairs*> lists;
+    double* d_scratch = nullptr;  // md4_compute_host staging
+    size_t scratch_doubles = 0;
+    long long launches = 0;
+    int num_sms = 0;
+    int smem_optin = 0;
+    md4::HostTables htab;
+};
+
+namespace md4 {
+// md4_pairs.cu
+cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t st);
+// md4_eri.cu
+md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
+                      cudaStream_t st);
+cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, double* d_out);
+cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out);
+}  // namespace md4

@@ -1,0 +1,90 @@
+"""CPU-side checks of the boundary: libmd4.so builds for sm_100a, loads, and exports every symbol that
+include/md4.h declares; the product path fails loudly without a CUDA device (no CPU fallback); the product
+package never imports the oracle.  No compute calls here."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "md4.h")
+
+
+def _declared():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(md4_[a-z_0-9]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2307_03452_b200 import build
+
+    path = build.build()
+    assert os.path.exists(path)
+    return ctypes.CDLL(path)
+
+
+def test_header_and_binding_agree():
+    from paper_2307_03452_b200 import md4
+
+    assert _declared() == sorted(md4.SYMBOLS)
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for name in _declared():
+        assert hasattr(lib, name), f"libmd4.so does not export {name}"
+
+
+def test_library_is_sm100a_with_fp64_mma():
+    """The built library carries sm_100a SASS and the contraction uses the FP64 tensor pipe (DMMA)."""
+    from paper_2307_03452_b200 import build
+
+    path = build.build()
+    r = subprocess.run(["cuobjdump", "-lelf", path], capture_output=True, text=True)
+    assert "sm_100a" in r.stdout, r.stdout + r.stderr
+    r = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True)
+    assert "DMMA.8x8x4" in r.stdout
+
+
+def test_no_cpu_fallback_without_gpu(lib):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2307_03452_b200 import md4
+
+    with pytest.raises(md4.Md4Error) as ei:
+        md4.Engine(0)
+    assert ei.value.status in (md4.MD4_ECUDA, md4.MD4_EINVAL)
+    assert md4.load().md4_last_error(None)
+
+
+def test_null_handles_are_rejected(lib):
+    lib.md4_set_shells.restype = ctypes.c_int
+    assert lib.md4_set_shells(None, 0, None, None, None, None, None) == 1
+    assert lib.md4_pairs_count(None) == -1
+    lib.md4_flops_per_quartet.restype = ctypes.c_double
+    assert lib.md4_flops_per_quartet(None, None) == 0.0
+    lib.md4_destroy(None)
+    lib.md4_free_pairs(None, None)
+    assert lib.md4_create(None, 0) == 1
+
+
+def test_product_never_imports_oracle():
+    pkg = os.path.join(ROOT, "paper_2307_03452_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "eri_oracle" not in txt, f
+    code = "import sys; import paper_2307_03452_b200.md4, paper_2307_03452_b200.inputs; assert 'oracle' not in sys.modules"
+    subprocess.run([sys.executable, "-c", code], check=True, cwd=ROOT)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "libmd4" not in txt and "import paper_2307_03452_b200" not in txt
