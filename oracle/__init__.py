@@ -1,7 +1,9 @@
 """CPU oracle for (ab|cd) -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
 
-Thin ctypes front end of ``oracle/eri_oracle.c`` (long-double Obara-Saika / Head-Gordon-Pople evaluator,
-SURVEY.md 8(c)).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+Thin ctypes front end of ``oracle/eri_oracle.c`` (Obara-Saika / Head-Gordon-Pople evaluator),
+built twice from the same source: ``liberi_oracle_q.so`` evaluates in IEEE binary128 and is the parity
+reference; ``liberi_oracle.so`` evaluates in x87 long double (the precision BASELINE.json names) and serves the
+cheap pins and the timed CPU baseline.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
 ``--impl reference`` legs may import this package.  It shares no code with ``paper_2307_03452_b200``
 and never imports it.
 """
@@ -66,7 +68,7 @@ def _bind(lib):
         lib.oracle_quartet_ld.argtypes = [d_p, i_p, i_p, d_p, d_p] + [ctypes.c_int] * 5 + [ld_p]
         lib.oracle_quartet_ld.restype = ctypes.c_int
         lib.oracle_compute.argtypes = [ctypes.c_int, d_p, i_p, i_p, d_p, d_p, ctypes.c_int, i_p, ctypes.c_int, i_p,
-                                       i_p, ctypes.c_int, d_p, ctypes.c_int]
+                                       i_p, ctypes.c_int, d_p, ctypes.c_int, ctypes.c_int]
         lib.oracle_compute.restype = ctypes.c_int
     return lib
 
@@ -138,9 +140,15 @@ def quartet(sh: Shells, ia: int, ib: int, ic: int, id_: int, solid: bool = True,
     return out
 
 
-def compute(sh: Shells, bra_ij, ket_ij, subset=None, nthreads: int | None = None) -> np.ndarray:
+def compute(sh: Shells, bra_ij, ket_ij, subset=None, nthreads: int | None = None, precision: str = "quad",
+            nslice: int = 1) -> np.ndarray:
     """Batch in the md4_compute layout, float64: out[i_bra, j_ket, ma, mb, mc, md]
-    (or out[k, ma, mb, mc, md] for the flat quartet indices i*nket+j listed in ``subset``)."""
+    (or out[k, ma, mb, mc, md] for the flat quartet indices i*nket+j listed in ``subset``).
+
+    precision: "quad" (default, the parity reference: IEEE binary128 build) or "ld" (x87 long-double build,
+    8x faster, loses up to ~1e-10 relative on tight high-l shells -- see the header of eri_oracle.c).
+    nslice > 1 spreads the primitive loop of each quartet over threads (heavily contracted quartets)."""
+    assert precision in ("quad", "ld")
     bra = np.ascontiguousarray(bra_ij, dtype=np.int32).reshape(-1, 2)
     ket = np.ascontiguousarray(ket_ij, dtype=np.int32).reshape(-1, 2)
     if nthreads is None:
@@ -155,9 +163,9 @@ def compute(sh: Shells, bra_ij, ket_ij, subset=None, nthreads: int | None = None
         sub = np.ascontiguousarray(subset, dtype=np.int32)
         out = np.zeros([sub.shape[0]] + dims, dtype=np.float64)
         sub_p, nsub = _i(sub), sub.shape[0]
-    rc = _load().oracle_compute(sh.l.shape[0], _d(sh.centers), _i(sh.l), _i(sh.prim_offset), _d(sh.exponents),
+    rc = _load(precision == "quad").oracle_compute(sh.l.shape[0], _d(sh.centers), _i(sh.l), _i(sh.prim_offset), _d(sh.exponents),
                                 _d(sh.coefficients), bra.shape[0], _i(bra), ket.shape[0], _i(ket), sub_p, nsub,
-                                _d(out), int(nthreads))
+                                _d(out), int(nthreads), int(nslice))
     if rc:
         raise RuntimeError(f"oracle_compute failed rc={rc}")
     return out

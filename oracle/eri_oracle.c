@@ -1,7 +1,7 @@
 /*
  * eri_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
  *
- * Plain, slow, long-double CPU evaluator of contracted 4-center 2-electron repulsion integrals
+ * Plain, slow, extended-precision CPU evaluator of contracted 4-center 2-electron repulsion integrals
  * (ab|cd) over real-solid-harmonic Gaussian shells.  It is the parity oracle for the CUDA path of
  * this repository and shares no code, header, table or constant with it.  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.
@@ -27,7 +27,18 @@
  *   4. contraction of the m = 0 values
  *   5. horizontal recurrence on contracted integrals
  *   6. 4-index Cartesian -> solid-harmonic transform
- * All arithmetic is long double (x87 80-bit on x86-64).
+ * Step 5 moves momentum away from the centre with the larger exponent, chosen per primitive pair (see
+ * quartet_cart): with a fixed direction the long-double result was wrong by 4e-3 on BASELINE config 1.
+ *
+ * Arithmetic type `real`.  Default build (liberi_oracle.so): long double (x87 80-bit on x86-64), the
+ * precision BASELINE.json names; it serves the pins and the timed CPU baseline.  -DORACLE_QUAD build
+ * (liberi_oracle_q.so): the same source in IEEE binary128 (libquadmath) -- THE PARITY REFERENCE.
+ * Why: step 6 projects Cartesian integrals onto solid harmonics; for a tight shell of high l far from its
+ * partner distribution the pure-l part is ~(s/R)^l of the Cartesian values (s = Gaussian width, R =
+ * distance), e.g. 1e-8..1e-9 for l = 6, and those digits are lost whatever the order of the steps.
+ * Measured on BASELINE config 3 (seeded sample of 10 quartets): long double vs binary128 differ by up to
+ * 7.6e-11 of max|integral| -- too close to the 1e-10 parity bar -- so parity is taken against binary128
+ * (error < 1e-24 by the same estimate).  Interfaces stay double / long double.
  */
 #include <math.h>
 #include <pthread.h>
@@ -35,8 +46,7 @@
 #include <string.h>
 
 #ifdef ORACLE_QUAD
-/* Audit build (liberi_oracle_q.so): the same source in IEEE binary128, used by tests only to measure
- * the rounding error of the long-double build on the hardest geometries.  Interfaces stay long double. */
+/* binary128 build (liberi_oracle_q.so): the parity reference, see the header. */
 #include <quadmath.h>
 typedef __float128 real;
 #define R_EXP expq
@@ -196,9 +206,18 @@ typedef struct {
     const double *exps, *coefs;
 } shell_t;
 
-static int quartet_cart(const shell_t *sa, const shell_t *sb, const shell_t *sc, const shell_t *sd, real *out)
+/* quartet_cart_dir: the part of the contraction whose primitive pairs have zeta_a >= zeta_b (zeta_a > zeta_b
+ * if strict_bra) and zeta_c >= zeta_d (zeta_c > zeta_d if strict_ket).  The vertical recurrence builds
+ * all momentum on the FIRST centre of each pair (A and C), the horizontal one moves it to the second.
+ * *nused = number of primitive quartets that passed the filter (0: out is not written).
+ * slice/nslice: only primitive quartets number slice, slice+nslice, ... of the four-fold loop are summed
+ * (the integral is linear in them; the batch driver adds the partial sums), nslice = 1 for everything.  */
+static int quartet_cart_dir(const shell_t *sa, const shell_t *sb, const shell_t *sc, const shell_t *sd,
+                            int strict_bra, int strict_ket, int slice, int nslice, real *out, int *nused)
 {
     pthread_once(&g_once, init_tables);
+    *nused = 0;
+    int prim_counter = 0;   /* primitive quartets are dealt round-robin to nslice independent partial sums */
     const int la = sa->l, lb = sb->l, lc = sc->l, ld = sd->l;
     const int lbra = la + lb, lket = lc + ld, L = lbra + lket;
     const int ne = ORACLE_NCUM(lbra + 1), nf = ORACLE_NCUM(lket + 1), nm = L + 1;
@@ -220,6 +239,10 @@ static int quartet_cart(const shell_t *sa, const shell_t *sb, const shell_t *sc,
     for (int kd = 0; kd < sd->nprim; ++kd) {
         /* step 1 */
         real za = sa->exps[ka], zb = sb->exps[kb], zc = sc->exps[kc], zd = sd->exps[kd];
+        if ((prim_counter++ % nslice) != slice) continue;
+        if (strict_bra ? !(za > zb) : !(za >= zb)) continue;
+        if (strict_ket ? !(zc > zd) : !(zc >= zd)) continue;
+        ++*nused;
         real p = za + zb, q = zc + zd, rho = p * q / (p + q);
         real P[3], Q[3], W[3], PA[3], QC[3], WP[3], WQ[3], PQ2 = 0;
         for (int i = 0; i < 3; ++i) {
@@ -272,6 +295,7 @@ static int quartet_cart(const shell_t *sa, const shell_t *sb, const shell_t *sc,
     }
 #undef VV
     free(V); free(F);
+    if (*nused == 0) { free(G); return 0; }
 
     /* step 5a, bra: (a,b+1_i| = (a+1_i,b| + (A_i-B_i)(a,b|, one ket index f at a time.
      * X[a*nbc + b], a over all degrees <= lbra, b over all degrees <= lb; keep |a| = la, |b| = lb.      */
@@ -312,6 +336,49 @@ static int quartet_cart(const shell_t *sa, const shell_t *sb, const shell_t *sc,
     return 0;
 }
 
+/* One contracted shell quartet, Cartesian components out[a][b][c][d] (steps 1-5).
+ *
+ * Direction of the horizontal recurrence.  (a,b+1_i| = (a+1_i,b| + (A_i-B_i)(a,b| rebuilds x_B^lb from
+ * powers of x_A; when the product Gaussian sits near B (zeta_b >> zeta_a, |P-A| ~ |AB|) the wanted value
+ * is small and the terms are of size |AB|^(la+lb): digits are lost (measured on BASELINE config 1:
+ * 4e-3 relative against the binary128 build of this file when A is always the building centre).
+ * The defining integral is symmetric, (ab|cd) = (ba|cd) = (ab|dc), so each primitive pair may build on
+ * either centre.  Here every primitive pair builds on its centre with the LARGER exponent, for which
+ * |P-A| <= |AB|/2 and the terms of the transfer are at most 3^lb times the result: the contraction is
+ * split into the four groups (zeta_a >= zeta_b | zeta_a < zeta_b) x (zeta_c >= zeta_d | zeta_c < zeta_d),
+ * each group goes through steps 1-5 with its own building centres, the swapped groups are transposed
+ * back, and the four Cartesian results are added.  Same recurrences, same result, no digits lost
+ * (reading R3).                                                                            */
+static int quartet_cart(const shell_t *sa, const shell_t *sb, const shell_t *sc, const shell_t *sd, int slice,
+                        int nslice, real *out)
+{
+    const int na = (sa->l + 1) * (sa->l + 2) / 2, nb = (sb->l + 1) * (sb->l + 2) / 2,
+              nc = (sc->l + 1) * (sc->l + 2) / 2, nd = (sd->l + 1) * (sd->l + 2) / 2;
+    const size_t n = (size_t)na * nb * nc * nd;
+    real *tmp = (real *)malloc(sizeof(real) * n);
+    if (!tmp) return 1;
+    for (size_t t = 0; t < n; ++t) out[t] = 0;
+    for (int swb = 0; swb < 2; ++swb)
+        for (int swk = 0; swk < 2; ++swk) {
+            int used = 0;
+            int rc = quartet_cart_dir(swb ? sb : sa, swb ? sa : sb, swk ? sd : sc, swk ? sc : sd, swb, swk, slice, nslice,
+                                      tmp, &used);
+            if (rc) { free(tmp); return rc; }
+            if (!used) continue;
+            /* tmp is [x0][x1][y0][y1] with (x0,x1) = (b,a) if swb and (y0,y1) = (d,c) if swk */
+            for (int a = 0; a < na; ++a)
+                for (int b = 0; b < nb; ++b)
+                    for (int c = 0; c < nc; ++c)
+                        for (int d = 0; d < nd; ++d) {
+                            size_t bra = swb ? (size_t)b * na + a : (size_t)a * nb + b;
+                            size_t ket = swk ? (size_t)d * nc + c : (size_t)c * nd + d;
+                            out[(((size_t)a * nb + b) * nc + c) * nd + d] += tmp[bra * ((size_t)nc * nd) + ket];
+                        }
+        }
+    free(tmp);
+    return 0;
+}
+
 /* step 6: transform one index of a 4-index array from Cartesian to solid harmonics.
  * in [n0][ncart][n2] -> out [n0][nsph][n2]                                                             */
 static void transform_index(const real *in, real *out, int n0, int l, int n2)
@@ -329,14 +396,15 @@ static void transform_index(const real *in, real *out, int n0, int l, int n2)
     free(C);
 }
 
-static int quartet_solid(const shell_t *sa, const shell_t *sb, const shell_t *sc, const shell_t *sd, real *out)
+static int quartet_solid(const shell_t *sa, const shell_t *sb, const shell_t *sc, const shell_t *sd, int slice,
+                         int nslice, real *out)
 {
     int l[4] = {sa->l, sb->l, sc->l, sd->l}, ncart[4], ns[4];
     size_t big = 1;
     for (int i = 0; i < 4; ++i) { ncart[i] = (l[i] + 1) * (l[i] + 2) / 2; ns[i] = 2 * l[i] + 1; big *= ncart[i]; }
     real *t0 = (real *)malloc(sizeof(real) * big), *t1 = (real *)malloc(sizeof(real) * big);
     if (!t0 || !t1) { free(t0); free(t1); return 1; }
-    int rc = quartet_cart(sa, sb, sc, sd, t0);
+    int rc = quartet_cart(sa, sb, sc, sd, slice, nslice, t0);
     if (!rc) {
         transform_index(t0, t1, 1, l[0], ncart[1] * ncart[2] * ncart[3]);
         transform_index(t1, t0, ns[0], l[1], ncart[2] * ncart[3]);
@@ -375,7 +443,8 @@ int oracle_quartet_ld(const double *centers, const int *l, const int *prim_offse
     for (int i = 0; i < 4; ++i) n *= solid ? (size_t)(2 * s[i].l + 1) : (size_t)((s[i].l + 1) * (s[i].l + 2) / 2);
     real *tmp = (real *)malloc(sizeof(real) * n);
     if (!tmp) return 1;
-    int rc = solid ? quartet_solid(&s[0], &s[1], &s[2], &s[3], tmp) : quartet_cart(&s[0], &s[1], &s[2], &s[3], tmp);
+    int rc = solid ? quartet_solid(&s[0], &s[1], &s[2], &s[3], 0, 1, tmp)
+                   : quartet_cart(&s[0], &s[1], &s[2], &s[3], 0, 1, tmp);
     for (size_t t = 0; t < n; ++t) out[t] = (long double)tmp[t];
     free(tmp);
     return rc;
@@ -386,38 +455,51 @@ typedef struct {
     int nbra; const int *bra_ij; int nket; const int *ket_ij;
     double *out; size_t per_quartet;
     const int *subset; int nsubset;         /* optional list of flat quartet indices i*nket+j */
+    int nslice; real *acc;                  /* nslice > 1: partial sums over primitive slices, added in acc */
     int next; pthread_mutex_t mu; int rc;
 } job_t;
 
 static void *worker(void *arg)
 {
     job_t *J = (job_t *)arg;
-    long double *buf = (long double *)malloc(sizeof(long double) * J->per_quartet);
-    int total = J->subset ? J->nsubset : J->nbra * J->nket;
+    real *buf = (real *)malloc(sizeof(real) * J->per_quartet);
+    int total = (J->subset ? J->nsubset : J->nbra * J->nket) * J->nslice;
     for (;;) {
         pthread_mutex_lock(&J->mu);
-        int k = J->next++;
+        int job = J->next++;
         pthread_mutex_unlock(&J->mu);
-        if (k >= total) break;
+        if (job >= total || !buf) break;
+        int k = job / J->nslice, slice = job % J->nslice;
         int flat = J->subset ? J->subset[k] : k;
         int i = flat / J->nket, j = flat % J->nket;
-        int rc = oracle_quartet_ld(J->centers, J->l, J->prim_offset, J->exps, J->coefs, J->bra_ij[2 * i],
-                                   J->bra_ij[2 * i + 1], J->ket_ij[2 * j], J->ket_ij[2 * j + 1], 1, buf);
-        if (rc) { J->rc = rc; break; }
+        shell_t s[4];
+        int idx[4] = {J->bra_ij[2 * i], J->bra_ij[2 * i + 1], J->ket_ij[2 * j], J->ket_ij[2 * j + 1]};
+        int rc = 0;
+        for (int t = 0; t < 4; ++t) rc |= make_shell(&s[t], idx[t], J->centers, J->l, J->prim_offset, J->exps, J->coefs);
+        if (!rc) rc = quartet_solid(&s[0], &s[1], &s[2], &s[3], slice, J->nslice, buf);
+        if (rc) { J->rc = rc ? rc : 2; break; }
         /* with a subset the k-th result goes to slot k, otherwise to slot i*nket+j */
-        double *dst = J->out + (size_t)(J->subset ? k : flat) * J->per_quartet;
-        for (size_t t = 0; t < J->per_quartet; ++t) dst[t] = (double)buf[t];
+        size_t slot = (size_t)(J->subset ? k : flat) * J->per_quartet;
+        if (J->nslice == 1) {
+            for (size_t t = 0; t < J->per_quartet; ++t) J->out[slot + t] = (double)buf[t];
+        } else {
+            pthread_mutex_lock(&J->mu);
+            for (size_t t = 0; t < J->per_quartet; ++t) J->acc[slot + t] += buf[t];
+            pthread_mutex_unlock(&J->mu);
+        }
     }
     free(buf);
     return NULL;
 }
 
-/* Batch: out[i_bra][j_ket][ma][mb][mc][md] (the layout of md4_compute, include/md4.h), rounded to
- * double.  All bra pairs must share (l_i,l_j), all ket pairs likewise.  If subset != NULL only the
- * listed flat quartet indices (i*nket + j) are computed and written densely: out[k][ma][mb][mc][md]. */
+/* Batch: out[i_bra][j_ket][ma][mb][mc][md] (the layout of md4_compute, include/md4.h), evaluated in `real`
+ * and rounded to double once at the end.  All bra pairs must share (l_i,l_j), all ket pairs likewise.  If
+ * subset != NULL only the listed flat quartet indices (i*nket + j) are computed and written densely:
+ * out[k][ma][mb][mc][md].  nslice > 1 splits the primitive loop of every quartet into nslice partial sums
+ * that run on different threads (for heavily contracted quartets); the partial sums are added in `real`. */
 int oracle_compute(int nshell, const double *centers, const int *l, const int *prim_offset, const double *exps,
                    const double *coefs, int nbra, const int *bra_ij, int nket, const int *ket_ij,
-                   const int *subset, int nsubset, double *out, int nthreads)
+                   const int *subset, int nsubset, double *out, int nthreads, int nslice)
 {
     (void)nshell;
     if (nbra <= 0 || nket <= 0) return 0;
@@ -426,7 +508,14 @@ int oracle_compute(int nshell, const double *centers, const int *l, const int *p
     J.centers = centers; J.l = l; J.prim_offset = prim_offset; J.exps = exps; J.coefs = coefs;
     J.nbra = nbra; J.bra_ij = bra_ij; J.nket = nket; J.ket_ij = ket_ij; J.out = out;
     J.subset = subset; J.nsubset = nsubset;
+    J.nslice = nslice < 1 ? 1 : nslice;
     J.per_quartet = (size_t)(2 * l[bra_ij[0]] + 1) * (2 * l[bra_ij[1]] + 1) * (2 * l[ket_ij[0]] + 1) * (2 * l[ket_ij[1]] + 1);
+    size_t nq = (size_t)(subset ? nsubset : nbra * nket);
+    if (J.nslice > 1) {
+        J.acc = (real *)malloc(sizeof(real) * nq * J.per_quartet);
+        if (!J.acc) return 1;
+        for (size_t t = 0; t < nq * J.per_quartet; ++t) J.acc[t] = 0;
+    }
     pthread_mutex_init(&J.mu, NULL);
     if (nthreads < 1) nthreads = 1;
     if (nthreads > 256) nthreads = 256;
@@ -434,5 +523,9 @@ int oracle_compute(int nshell, const double *centers, const int *l, const int *p
     for (int t = 0; t < nthreads; ++t) pthread_create(&th[t], NULL, worker, &J);
     for (int t = 0; t < nthreads; ++t) pthread_join(th[t], NULL);
     pthread_mutex_destroy(&J.mu);
+    if (J.nslice > 1) {
+        if (!J.rc) for (size_t t = 0; t < nq * J.per_quartet; ++t) out[t] = (double)J.acc[t];
+        free(J.acc);
+    }
     return J.rc;
 }

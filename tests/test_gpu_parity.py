@@ -9,6 +9,7 @@ import numpy as np
 import pytest
 
 import oracle
+from mpmd import mp_H as _mp_H, mp_R as _mp_R
 from paper_2307_03452_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -97,45 +98,6 @@ def test_solid_coeff_stage(eng):
         assert np.abs(got - ref).max() <= 1e-14 * max(1.0, np.abs(ref).max()), l
 
 
-def _mp_R(L, zp, P, zq, Q):
-    import mpmath as mp
-
-    mp.mp.dps = 40
-    zp, zq = mp.mpf(zp), mp.mpf(zq)
-    X = [mp.mpf(float(a)) - mp.mpf(float(b)) for a, b in zip(P, Q)]
-    rho = zp * zq / (zp + zq)
-    T = rho * sum(x * x for x in X)
-    pref = 2 * mp.pi ** mp.mpf(2.5) / (zp * zq * mp.sqrt(zp + zq))
-
-    def F(m):
-        if T == 0:
-            return mp.mpf(1) / (2 * m + 1)
-        return mp.gammainc(m + mp.mpf(1) / 2, 0, T) / (2 * T ** (m + mp.mpf(1) / 2))
-
-    # R[m][(t,u,v)], Helgaker-style: R^m_{t+1} = t R^{m+1}_{t-1} + X R^{m+1}_t  (Eq.13)
-    R = {}
-    for m in range(L + 1):
-        R[(m, 0, 0, 0)] = pref * (-2 * rho) ** m * F(m)
-    for n in range(1, L + 1):
-        for t in range(n + 1):
-            for u in range(n - t + 1):
-                v = n - t - u
-                for m in range(L - n + 1):
-                    if t > 0:
-                        val = X[0] * R[(m + 1, t - 1, u, v)] + ((t - 1) * R[(m + 1, t - 2, u, v)] if t > 1 else 0)
-                    elif u > 0:
-                        val = X[1] * R[(m + 1, t, u - 1, v)] + ((u - 1) * R[(m + 1, t, u - 2, v)] if u > 1 else 0)
-                    else:
-                        val = X[2] * R[(m + 1, t, u, v - 1)] + ((v - 1) * R[(m + 1, t, u, v - 2)] if v > 1 else 0)
-                    R[(m, t, u, v)] = val
-    out = np.zeros((L + 1,) * 3)
-    for t in range(L + 1):
-        for u in range(L + 1 - t):
-            for v in range(L + 1 - t - u):
-                out[t, u, v] = float(R[(0, t, u, v)])
-    return out
-
-
 @pytest.mark.parametrize("L,zp,zq,P,Q", [
     (24, 1.7, 0.9, (0.1, 0.2, -0.3), (1.0, -0.7, 0.45)),
     (24, 30.0, 45.0, (0.0, 0.0, 0.0), (3.0, 4.0, 5.0)),       # large T: asymptotic branch
@@ -151,45 +113,6 @@ def test_hermite_r_stage(eng, L, zp, zq, P, Q):
         idx = [(t, u, n - t - u) for t in range(n + 1) for u in range(n - t + 1)]
         r = np.array([ref[i] for i in idx]); g = np.array([got[i] for i in idx])
         assert np.abs(g - r).max() <= R_STAGE_TOL * np.abs(r).max(), (n, np.abs(g - r).max() / np.abs(r).max())
-
-
-def _mp_H(sh, i, j, ka, kb):
-    """H = c_a c_b C_la (x) C_lb E for one primitive pair, 40-digit E by Eq.4-5, oracle's solid tables."""
-    import mpmath as mp
-
-    mp.mp.dps = 40
-    li, lj = int(sh.l[i]), int(sh.l[j])
-    za = mp.mpf(float(sh.exponents[sh.prim_offset[i] + ka])); zb = mp.mpf(float(sh.exponents[sh.prim_offset[j] + kb]))
-    ca = mp.mpf(float(sh.coefficients[sh.prim_offset[i] + ka])); cb = mp.mpf(float(sh.coefficients[sh.prim_offset[j] + kb]))
-    A = [mp.mpf(float(x)) for x in sh.centers[i]]; B = [mp.mpf(float(x)) for x in sh.centers[j]]
-    p = za + zb
-    P = [(za * a + zb * b) / p for a, b in zip(A, B)]
-    E = []
-    for ax in range(3):
-        e = {(0, 0, 0): mp.mpf(1)}
-        g = lambda a_, b_, t_: e.get((a_, b_, t_), mp.mpf(0))
-        for a_ in range(li):
-            for t in range(a_ + 2):
-                e[(a_ + 1, 0, t)] = g(a_, 0, t - 1) / (2 * p) + (P[ax] - A[ax]) * g(a_, 0, t) + (t + 1) * g(a_, 0, t + 1)
-        for a_ in range(li + 1):
-            for b_ in range(lj):
-                for t in range(a_ + b_ + 2):
-                    e[(a_, b_ + 1, t)] = g(a_, b_, t - 1) / (2 * p) + (P[ax] - B[ax]) * g(a_, b_, t) + (t + 1) * g(a_, b_, t + 1)
-        E.append(e)
-    Ca, Cb = oracle.solid_coeff(li), oracle.solid_coeff(lj)
-    carta, cartb = oracle.cart_list(li), oracle.cart_list(lj)
-    lb = li + lj
-    herm = [(t, u, n - t - u) for n in range(lb + 1) for t in range(n, -1, -1) for u in range(n - t, -1, -1)]
-    Ecart = np.zeros((len(carta), len(cartb), len(herm)), dtype=object)
-    for ia, a in enumerate(carta):
-        for ib, b in enumerate(cartb):
-            for ih, (t, u, v) in enumerate(herm):
-                Ecart[ia, ib, ih] = (E[0].get((a[0], b[0], t), 0) * E[1].get((a[1], b[1], u), 0) * E[2].get((a[2], b[2], v), 0))
-    Ecart = np.array(Ecart, dtype=np.longdouble)
-    H = np.einsum("ma,nb,abh->mnh", Ca, Cb, Ecart) * np.longdouble(float(ca * cb))
-    mu = za * zb / p
-    lnK = -mu * sum((a - b) ** 2 for a, b in zip(A, B))
-    return H.reshape(-1, len(herm)).astype(np.float64), float(p), [float(x) for x in P], float(lnK)
 
 
 @pytest.mark.parametrize("lclass,kclass", [((2, 1, 0, 0), (1, 1, 1, 1)), ((4, 3, 0, 0), (2, 1, 1, 1)), ((6, 6, 0, 0), (1, 1, 1, 1))])

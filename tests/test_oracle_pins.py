@@ -294,3 +294,59 @@ def test_paper_size_statements():
     assert I.class_flops((6, 6, 6, 6), (1, 1, 1, 1)) == 95964960
     assert I.class_flops((6, 6, 6, 6), (5, 5, 5, 5)) == 44383794000
     assert I.class_flops((4, 4, 4, 4), (1, 1, 1, 1)) == 6575580
+
+
+# ------------------------------------------------- hard geometries: tight/diffuse pairs far from their partners
+def _config1_shells():
+    from paper_2307_03452_b200 import inputs as I
+
+    wl = I.config1()
+    s = wl.shells
+    return oracle.Shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+
+
+def test_hard_geometry_vs_40_digit_md():
+    """BASELINE config 1, bra (0,1) x ket (5,4): zeta = (0.156, 8.24 | 0.136, 10.4), |CD| = 6.5 bohr, T = 215.
+    With the horizontal recurrence always moving momentum from the first to the second centre the long-double
+    oracle was wrong by 4e-3 here.  Reference: the paper's MD form at 40 digits (tests/mpmd.py), a third route."""
+    import mpmd
+
+    sh = _config1_shells()
+    rows = [(0, 0), (4, 4), (8, 1), (3, 7), (6, 2)]
+    ref = mpmd.mp_quartet_rows(sh, 0, 1, 5, 4, rows)
+    for quad, tol in ((True, 1e-15), (False, 1e-11)):
+        q = oracle.quartet(sh, 0, 1, 5, 4, quad=quad).astype(np.float64)
+        got = np.stack([q[a, b] for a, b in rows])
+        assert np.abs(got - ref).max() <= tol * np.abs(q).max(), (quad, np.abs(got - ref).max() / np.abs(q).max())
+
+
+def test_building_centre_choice_is_symmetric():
+    """(ab|cd) = (ba|cd) = (cd|ab) on a hard geometry, in both builds; equal exponents (tie) included."""
+    cent = [[0, 0, 0], [0, 0, 5.0], [4.0, 1.0, 0], [4.0, 1.0, 0.7]]
+    for zs in ([0.12, 9.0, 11.0, 0.2], [0.5, 0.5, 3.0, 3.0]):
+        sh = oracle.Shells(cent, [4, 3, 3, 4], [0, 1, 2, 3, 4], zs, [1, 1, 1, 1])
+        for quad, tol in ((True, 1e-25), (False, 1e-12)):
+            q = oracle.quartet(sh, 0, 1, 2, 3, quad=quad)
+            mx = np.abs(q).max()
+            assert np.abs(oracle.quartet(sh, 2, 3, 0, 1, quad=quad) - q.transpose(2, 3, 0, 1)).max() <= max(tol, 2e-18) * mx
+            assert np.abs(oracle.quartet(sh, 1, 0, 3, 2, quad=quad) - q.transpose(1, 0, 3, 2)).max() <= max(tol, 2e-18) * mx
+
+
+def test_batch_driver_slices_and_precisions():
+    """oracle.compute: primitive slices add up to the unsliced result; binary128 and long-double builds agree on a
+    benign contracted geometry; subset addressing."""
+    rng = np.random.default_rng(77)
+    sh = _rand_shells(rng, [2, 1, 2, 1], K=(3, 2, 2, 3))
+    bra, ket = np.array([[0, 1], [1, 0]], dtype=np.int32), np.array([[2, 3]], dtype=np.int32)
+    sh2 = oracle.Shells(np.concatenate([sh.centers]), sh.l, sh.prim_offset, sh.exponents, sh.coefficients)
+    # bra pair (1,0) has (l1,l0) = (1,2): lists must share a class, so use two lists of one pair each
+    for b in (bra[:1], bra[1:]):
+        full = oracle.compute(sh2, b, ket, nthreads=2)
+        sliced = oracle.compute(sh2, b, ket, nthreads=3, nslice=5)
+        ld = oracle.compute(sh2, b, ket, nthreads=2, precision="ld")
+        assert np.abs(full - sliced).max() <= 1e-16 * np.abs(full).max()
+        assert np.abs(full - ld).max() <= 1e-15 * np.abs(full).max()
+        one = oracle.quartet(sh2, int(b[0, 0]), int(b[0, 1]), 2, 3, quad=True).astype(np.float64)
+        assert np.array_equal(full[0, 0], one)
+        sub = oracle.compute(sh2, b, ket, subset=[0], nthreads=1)
+        assert np.array_equal(sub[0], full[0, 0])
