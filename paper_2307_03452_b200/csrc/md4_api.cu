@@ -81,6 +81,10 @@ md4_status md4_create(md4_ctx** out, int cuda_device) {
         double* d = nullptr;
         e = upload(&c->table_allocs, c->htab.solid[l].data(), c->htab.solid[l].size(), &d);
         c->tab.solid[l] = d;
+        if (e == cudaSuccess) {
+            e = upload(&c->table_allocs, c->htab.solid_lo[l].data(), c->htab.solid_lo[l].size(), &d);
+            c->tab.solid_lo[l] = d;
+        }
     }
     if (e != cudaSuccess) {
         g_create_err = std::string("md4_create: table upload: ") + cudaGetErrorString(e);

@@ -39,13 +39,14 @@ struct DeviceTables {
     const uint32_t* rtab;    // [NR_MAX] packed {idx0:12, idx1:12, C:5, axis:2} of Eq.13
     const uint32_t* tuv;     // [NR_MAX] packed t | u << 8 | v << 16 in graded order
     const double* boys;      // [BOYS_NODES * BOYS_STRIDE]
-    const double* solid[LMAX + 1];  // [(2l+1) * n_cart(l)]
+    const double* solid[LMAX + 1];     // [(2l+1) * n_cart(l)]  high parts
+    const double* solid_lo[LMAX + 1];  // low parts of the double-double coefficients
 };
 
 struct HostTables {
     std::vector<uint32_t> rtab, tuv;
     std::vector<double> boys;
-    std::vector<double> solid[LMAX + 1];
+    std::vector<double> solid[LMAX + 1], solid_lo[LMAX + 1];
 };
 void build_host_tables(HostTables& t);  // md4_tables.cpp
 

@@ -2,7 +2,8 @@
 // compute_hermite_gaussian_transform, Listing 2.1 lines 2-3).
 // Per primitive pair: zeta_p, R_p, ln K_ab (S:8(c) Q2), the 1-D Hermite expansion tables
 // (E_i)^t_{a_i b_i} by Eq.4-5, and H = c_a c_b C_la (x) C_lb E (Eq.16) as two
-// half transforms, written in the 8x8-blocked layout of md4_internal.h.
+// half transforms in double-double arithmetic, rounded to FP64 and written in the 8x8-blocked layout of
+// md4_internal.h.
 #include "md4_internal.h"
 
 namespace md4 {
@@ -13,6 +14,42 @@ constexpr int NT1 = 2 * LMAX + 1;      // t = 0..12
 constexpr int ESZ = NA1 * NA1 * NT1;   // 637 per axis
 constexpr int NCMAX = (LMAX + 1) * (LMAX + 2) / 2;  // 28
 constexpr int NSMAX = 2 * LMAX + 1;    // 13
+constexpr int PAIR_THREADS = 256;
+constexpr int PAIR_SPLIT = 4;          // CTAs per primitive pair (each takes a range of Hermite column blocks)
+
+// ---- double-double arithmetic (error-free transformations; __d*_rn blocks FMA contraction) ---------
+// Why: H = C_la (x) C_lb E cancels the radial contaminants of the Cartesian Gaussians.  For a tight
+// shell of high l far from its partner the surviving part is ~(2 zeta_p)^-l/2 of the terms (1e-6 for
+// l = 6, zeta_p = 50) and it meets R values that are ~R^6/720 larger than the ones the leading part
+// meets: in plain FP64 the error reached 3e-8 of max|integral| on BASELINE config 5 (bar 1e-10).
+// E, the E products and both half transforms therefore run in double-double; H is rounded to FP64 at
+// the end, every entry correct to ~1e-16 of ITSELF.
+typedef double2 dd;  // x = hi, y = lo
+__device__ __forceinline__ dd dd_two_sum(double a, double b) {
+    const double s = __dadd_rn(a, b), bb = __dadd_rn(s, -a);
+    return make_double2(s, __dadd_rn(__dadd_rn(a, -__dadd_rn(s, -bb)), __dadd_rn(b, -bb)));
+}
+__device__ __forceinline__ dd dd_quick(double a, double b) {
+    const double s = __dadd_rn(a, b);
+    return make_double2(s, __dadd_rn(b, -__dadd_rn(s, -a)));
+}
+__device__ __forceinline__ dd dd_add(dd a, dd b) {
+    dd s = dd_two_sum(a.x, b.x);
+    return dd_quick(s.x, __dadd_rn(s.y, __dadd_rn(a.y, b.y)));
+}
+__device__ __forceinline__ dd dd_mul(dd a, dd b) {
+    const double p = __dmul_rn(a.x, b.x);
+    double e = __fma_rn(a.x, b.x, -p);
+    e = __fma_rn(a.x, b.y, e);
+    e = __fma_rn(a.y, b.x, e);
+    return dd_quick(p, e);
+}
+__device__ __forceinline__ dd dd_mul_d(dd a, double b) {
+    const double p = __dmul_rn(a.x, b);
+    double e = __fma_rn(a.x, b, -p);
+    e = __fma_rn(a.y, b, e);
+    return dd_quick(p, e);
+}
 
 struct PairKernelArgs {
     const double* centers;
@@ -21,24 +58,29 @@ struct PairKernelArgs {
     const double* coef;
     const int* ij;
     const uint32_t* tuv;
-    const double* Ca;  // [(2li+1) * nc(li)]
-    const double* Cb;
+    const double *Ca, *CaLo;  // [(2li+1) * nc(li)] high / low parts
+    const double *Cb, *CbLo;
     double* H;
     double* scal;
     int li, lj, Ki, Kj, nab, nrb, nherm, ncb;
     size_t hstride;
 };
 
-__global__ void __launch_bounds__(256) pair_h_kernel(PairKernelArgs a) {
-    __shared__ double sE[3][ESZ];
-    __shared__ double sCa[NSMAX * NCMAX];
-    __shared__ double sCb[NSMAX * NCMAX];
-    __shared__ double sY[NCMAX * NSMAX * 8];
-    __shared__ unsigned char sca[NCMAX][2], scb[NCMAX][2];
+struct PairSmem {
+    dd E[3][ESZ];
+    dd Ca[NSMAX * NCMAX];
+    dd Cb[NSMAX * NCMAX];
+    dd Y[NCMAX * NSMAX * 8];
+    unsigned char ca[NCMAX][2], cb[NCMAX][2];
+};
+
+__global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) {
+    extern __shared__ __align__(16) unsigned char pair_smem_raw[];
+    PairSmem& sm = *reinterpret_cast<PairSmem*>(pair_smem_raw);
 
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int jb = blockIdx.x % a.ncb;
-    const int ip = blockIdx.x / a.ncb;
+    const int split = blockIdx.x % PAIR_SPLIT;
+    const int ip = blockIdx.x / PAIR_SPLIT;
     const int kk = a.Ki * a.Kj;
     const int ipair = ip / kk, kab = ip % kk, ka = kab / a.Kj, kb = kab % a.Kj;
     const int si = a.ij[2 * ipair], sj = a.ij[2 * ipair + 1];
@@ -47,26 +89,30 @@ __global__ void __launch_bounds__(256) pair_h_kernel(PairKernelArgs a) {
 
     const double za = a.expo[a.off[si] + ka], zb = a.expo[a.off[sj] + kb];
     const double zp = za + zb;
-    double A[3], B[3], P[3];
+    double A[3], B[3], P[3], XPA[3], XPB[3];
     double ab2 = 0.0;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         A[i] = a.centers[3 * si + i];
         B[i] = a.centers[3 * sj + i];
+        const double d = B[i] - A[i];
         P[i] = (za * A[i] + zb * B[i]) / zp;
-        ab2 += (A[i] - B[i]) * (A[i] - B[i]);
+        // P - A and P - B from the centre difference: each keeps full relative accuracy when P sits on a centre
+        XPA[i] = (zb / zp) * d;
+        XPB[i] = -(za / zp) * d;
+        ab2 += d * d;
     }
-    for (int i = tid; i < 3 * ESZ; i += nthr) (&sE[0][0])[i] = 0.0;
-    for (int i = tid; i < nsa * nca; i += nthr) sCa[i] = a.Ca[i];
-    for (int i = tid; i < nsb * ncbt; i += nthr) sCb[i] = a.Cb[i];
+    for (int i = tid; i < 3 * ESZ; i += nthr) (&sm.E[0][0])[i] = make_double2(0.0, 0.0);
+    for (int i = tid; i < nsa * nca; i += nthr) sm.Ca[i] = make_double2(a.Ca[i], a.CaLo[i]);
+    for (int i = tid; i < nsb * ncbt; i += nthr) sm.Cb[i] = make_double2(a.Cb[i], a.CbLo[i]);
     if (tid == 0) {
         int k = 0;
         for (int x = li; x >= 0; --x)
-            for (int y = li - x; y >= 0; --y, ++k) { sca[k][0] = x; sca[k][1] = y; }
+            for (int y = li - x; y >= 0; --y, ++k) { sm.ca[k][0] = x; sm.ca[k][1] = y; }
         k = 0;
         for (int x = lj; x >= 0; --x)
-            for (int y = lj - x; y >= 0; --y, ++k) { scb[k][0] = x; scb[k][1] = y; }
-        if (jb == 0) {
+            for (int y = lj - x; y >= 0; --y, ++k) { sm.cb[k][0] = x; sm.cb[k][1] = y; }
+        if (split == 0) {
             double* s = a.scal + (size_t)ip * 8;
             s[0] = zp; s[1] = P[0]; s[2] = P[1]; s[3] = P[2];
             s[4] = -(za * zb / zp) * ab2;  // ln K_ab; made relative to the pair maximum by pair_finalize_kernel
@@ -74,58 +120,74 @@ __global__ void __launch_bounds__(256) pair_h_kernel(PairKernelArgs a) {
         }
     }
     __syncthreads();
-    // 1-D tables, one thread per axis (Eq.4: raise a at b = 0, Eq.5: raise b), seed (E_i)^0_00 = 1.
-    if (tid < 3) {
-        double* E = sE[tid];
-        const double xpa = P[tid] - A[tid], xpb = P[tid] - B[tid], h = 0.5 / zp;
-        E[0] = 1.0;
-        for (int ai = 0; ai < li; ++ai)
-            for (int t = 0; t <= ai + 1; ++t) {
-                const double* e = E + (ai * NA1) * NT1;
-                double v = xpa * e[t];
-                if (t < ai) v += (t + 1) * e[t + 1];  // (E)^t_ab = 0 for t > a+b
-                if (t > 0) v += h * e[t - 1];
+    // 1-D tables (Eq.4: raise a at b = 0, Eq.5: raise b), seed (E_i)^0_00 = 1: warp i does axis i,
+    // lane t does Hermite order t; one step of the recurrence per __syncwarp.
+    const int warp = tid >> 5, lane = tid & 31;
+    if (warp < 3) {
+        dd* E = sm.E[warp];
+        const double xpa = XPA[warp], xpb = XPB[warp], h = 0.5 / zp;
+        if (lane == 0) E[0] = make_double2(1.0, 0.0);
+        __syncwarp();
+        for (int ai = 0; ai < li; ++ai) {
+            const dd* e = E + (ai * NA1) * NT1;
+            const int t = lane;
+            if (t <= ai + 1) {
+                dd v = dd_mul_d(e[t], xpa);
+                if (t < ai) v = dd_add(v, dd_mul_d(e[t + 1], (double)(t + 1)));  // (E)^t_ab = 0 for t > a+b
+                if (t > 0) v = dd_add(v, dd_mul_d(e[t - 1], h));
                 E[((ai + 1) * NA1) * NT1 + t] = v;
             }
-        for (int ai = 0; ai <= li; ++ai)
-            for (int bi = 0; bi < lj; ++bi)
-                for (int t = 0; t <= ai + bi + 1; ++t) {
-                    const double* e = E + (ai * NA1 + bi) * NT1;
-                    double v = xpb * e[t];
-                    if (t < ai + bi) v += (t + 1) * e[t + 1];
-                    if (t > 0) v += h * e[t - 1];
+            __syncwarp();
+        }
+        for (int bi = 0; bi < lj; ++bi) {
+            // all a_i in parallel: lanes (ai, t) flattened
+            for (int idx = lane; idx < (li + 1) * NT1; idx += 32) {
+                const int ai = idx / NT1, t = idx % NT1;
+                if (t <= ai + bi + 1) {
+                    const dd* e = E + (ai * NA1 + bi) * NT1;
+                    dd v = dd_mul_d(e[t], xpb);
+                    if (t < ai + bi) v = dd_add(v, dd_mul_d(e[t + 1], (double)(t + 1)));
+                    if (t > 0) v = dd_add(v, dd_mul_d(e[t - 1], h));
                     E[(ai * NA1 + bi + 1) * NT1 + t] = v;
                 }
-    }
-    __syncthreads();
-    // half transform over b: Y[ac][mb][pp] = sum_bc Cb[mb][bc] Ex Ey Ez
-    for (int idx = tid; idx < nca * nsb * 8; idx += nthr) {
-        const int pp = idx & 7, mb = (idx >> 3) % nsb, ac = (idx >> 3) / nsb;
-        const int col = jb * 8 + pp;
-        double acc = 0.0;
-        if (col < a.nherm) {
-            const uint32_t w = a.tuv[col];
-            const int t = w & 255, u = (w >> 8) & 255, v = (w >> 16) & 255;
-            const int ax = sca[ac][0], ay = sca[ac][1], az = li - ax - ay;
-            for (int bc = 0; bc < ncbt; ++bc) {
-                const int bx = scb[bc][0], by = scb[bc][1], bz = lj - bx - by;
-                if (t > ax + bx || u > ay + by || v > az + bz) continue;
-                acc += sCb[mb * ncbt + bc] * (sE[0][(ax * NA1 + bx) * NT1 + t] * sE[1][(ay * NA1 + by) * NT1 + u] *
-                                              sE[2][(az * NA1 + bz) * NT1 + v]);
             }
+            __syncwarp();
         }
-        sY[idx] = acc;
     }
     __syncthreads();
-    // half transform over a, contraction weight, blocked store
     const double wgt = a.coef[a.off[si] + ka] * a.coef[a.off[sj] + kb];
-    double* Hp = a.H + (size_t)ip * a.hstride + (size_t)jb * a.nrb * 64;
-    for (int idx = tid; idx < a.nab * 8; idx += nthr) {
-        const int pp = idx & 7, row = idx >> 3;
-        const int ma = row / nsb, mb = row % nsb;
-        double acc = 0.0;
-        for (int ac = 0; ac < nca; ++ac) acc += sCa[ma * nca + ac] * sY[(ac * nsb + mb) * 8 + pp];
-        Hp[(row >> 3) * 64 + (row & 7) * 8 + pp] = wgt * acc;
+    const int jb0 = (int)((long long)split * a.ncb / PAIR_SPLIT), jb1 = (int)((long long)(split + 1) * a.ncb / PAIR_SPLIT);
+    for (int jb = jb0; jb < jb1; ++jb) {
+        // half transform over b: Y[ac][mb][pp] = sum_bc Cb[mb][bc] Ex Ey Ez
+        for (int idx = tid; idx < nca * nsb * 8; idx += nthr) {
+            const int pp = idx & 7, mb = (idx >> 3) % nsb, ac = (idx >> 3) / nsb;
+            const int col = jb * 8 + pp;
+            dd acc = make_double2(0.0, 0.0);
+            if (col < a.nherm) {
+                const uint32_t w = a.tuv[col];
+                const int t = w & 255, u = (w >> 8) & 255, v = (w >> 16) & 255;
+                const int ax = sm.ca[ac][0], ay = sm.ca[ac][1], az = li - ax - ay;
+                for (int bc = 0; bc < ncbt; ++bc) {
+                    const int bx = sm.cb[bc][0], by = sm.cb[bc][1], bz = lj - bx - by;
+                    if (t > ax + bx || u > ay + by || v > az + bz) continue;
+                    const dd e3 = dd_mul(dd_mul(sm.E[0][(ax * NA1 + bx) * NT1 + t], sm.E[1][(ay * NA1 + by) * NT1 + u]),
+                                         sm.E[2][(az * NA1 + bz) * NT1 + v]);
+                    acc = dd_add(acc, dd_mul(sm.Cb[mb * ncbt + bc], e3));
+                }
+            }
+            sm.Y[idx] = acc;
+        }
+        __syncthreads();
+        // half transform over a, contraction weight, blocked store
+        double* Hp = a.H + (size_t)ip * a.hstride + (size_t)jb * a.nrb * 64;
+        for (int idx = tid; idx < a.nab * 8; idx += nthr) {
+            const int pp = idx & 7, row = idx >> 3;
+            const int ma = row / nsb, mb = row % nsb;
+            dd acc = make_double2(0.0, 0.0);
+            for (int ac = 0; ac < nca; ++ac) acc = dd_add(acc, dd_mul(sm.Ca[ma * nca + ac], sm.Y[(ac * nsb + mb) * 8 + pp]));
+            Hp[(row >> 3) * 64 + (row & 7) * 8 + pp] = wgt * acc.x + wgt * acc.y;
+        }
+        __syncthreads();
     }
 }
 
@@ -147,13 +209,17 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
     if (e != cudaSuccess) return e;
     PairKernelArgs a;
     a.centers = ctx->d_centers; a.off = ctx->d_off; a.expo = ctx->d_exp; a.coef = ctx->d_coef;
-    a.ij = pl.ij; a.tuv = ctx->tab.tuv; a.Ca = ctx->tab.solid[pl.li]; a.Cb = ctx->tab.solid[pl.lj];
+    a.ij = pl.ij; a.tuv = ctx->tab.tuv;
+    a.Ca = ctx->tab.solid[pl.li]; a.CaLo = ctx->tab.solid_lo[pl.li];
+    a.Cb = ctx->tab.solid[pl.lj]; a.CbLo = ctx->tab.solid_lo[pl.lj];
     a.H = pl.H; a.scal = pl.scal;
     a.li = pl.li; a.lj = pl.lj; a.Ki = pl.Ki; a.Kj = pl.Kj;
     a.nab = pl.nab; a.nrb = pl.nrb; a.nherm = pl.nherm; a.ncb = pl.ncb; a.hstride = pl.hstride;
-    const size_t nblk = nprim * pl.ncb;
+    const size_t nblk = nprim * PAIR_SPLIT;
     if (nblk > 2147483647ull) return cudaErrorInvalidValue;
-    pair_h_kernel<<<(unsigned)nblk, 256, 0, st>>>(a);
+    e = cudaFuncSetAttribute(pair_h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PairSmem));
+    if (e != cudaSuccess) return e;
+    pair_h_kernel<<<(unsigned)nblk, PAIR_THREADS, sizeof(PairSmem), st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

@@ -16,11 +16,14 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-10
 FLOOR = 1e-280
-# Stage bar for R (S:8(a) a4): the level recurrence Eq.13 runs L <= 24 levels in FP64 and each entry is a
-# signed sum over recurrence paths (multipole-like polynomials in X_PQ), so rounding is amplified by the
-# cancellation between paths: measured 4.5e-13 of the per-degree maximum at L = 24, T = 900.  The bar is
-# set a decade below the end-to-end 1e-10.
-R_STAGE_TOL = 1e-11
+# Stage bar for R (S:8(a) a4).  The level recurrence Eq.13 adds two terms of opposite sign at every step; in the
+# multipole limit (large T) the seeds are (-1)^m (2m-1)!!/r^(2m+1) and the result of degree n is ~ n!/r^(n+1), so
+# the recurrence is conditioned like (2n-1)!!/n! = C(2n,n)/2^n (2.6e5 at n = 21, 1.9e6 at n = 24): any FP64
+# evaluation of Eq.13 carries that factor times 2^-53 (measured on B200: 2.1e-11 of the per-degree maximum at
+# n = 21, T = 900).  The high degrees meet E coefficients ~(1/2p)^t in the contraction, so the end-to-end bar of
+# 1e-10 is unaffected (checked by the config tests).  Bar per degree: 4 * 2^-53 * C(2n,n)/2^n + 1e-13.
+def _r_stage_tol(n):
+    return 4.0 * 2.0 ** -53 * math.comb(2 * n, n) / 2.0 ** n + 1e-13
 
 
 @pytest.fixture(scope="module")
@@ -55,8 +58,8 @@ def _quartet_errors(gpu, ref):
     return np.array(errs), below
 
 
-def _run(eng, wl, subset=None):
-    """Full batch on the GPU; oracle on all quartets or on the flat indices in `subset`."""
+def _run(eng, wl, subset=None, nslice=1):
+    """Full batch on the GPU; oracle (binary128 build) on all quartets or on the flat indices in `subset`."""
     import torch
 
     s = wl.shells
@@ -69,11 +72,11 @@ def _run(eng, wl, subset=None):
     nb, nk = g.shape[:2]
     g = g.reshape((nb * nk,) + g.shape[2:])
     if subset is None:
-        ref = oracle.compute(_oshells(s), wl.bra_ij, wl.ket_ij)
+        ref = oracle.compute(_oshells(s), wl.bra_ij, wl.ket_ij, nslice=nslice)
         ref = ref.reshape(g.shape)
         return g, ref
     sub = np.asarray(subset, dtype=np.int32)
-    ref = oracle.compute(_oshells(s), wl.bra_ij, wl.ket_ij, subset=sub)
+    ref = oracle.compute(_oshells(s), wl.bra_ij, wl.ket_ij, subset=sub, nslice=nslice)
     return g[sub], ref
 
 
@@ -112,7 +115,7 @@ def test_hermite_r_stage(eng, L, zp, zq, P, Q):
     for n in range(L + 1):
         idx = [(t, u, n - t - u) for t in range(n + 1) for u in range(n - t + 1)]
         r = np.array([ref[i] for i in idx]); g = np.array([got[i] for i in idx])
-        assert np.abs(g - r).max() <= R_STAGE_TOL * np.abs(r).max(), (n, np.abs(g - r).max() / np.abs(r).max())
+        assert np.abs(g - r).max() <= _r_stage_tol(n) * np.abs(r).max(), (n, np.abs(g - r).max() / np.abs(r).max())
 
 
 @pytest.mark.parametrize("lclass,kclass", [((2, 1, 0, 0), (1, 1, 1, 1)), ((4, 3, 0, 0), (2, 1, 1, 1)), ((6, 6, 0, 0), (1, 1, 1, 1))])
@@ -168,10 +171,10 @@ def test_config1_full(eng):
     assert errs.max() <= TOL, errs.max()
 
 
-def _sampled(eng, wl, nsample, seed, extra=()):
+def _sampled(eng, wl, nsample, seed, extra=(), nslice=1):
     rng = np.random.Generator(np.random.PCG64(seed))
     sub = np.unique(np.concatenate([rng.choice(wl.nquartets, size=nsample, replace=False), np.asarray(extra, dtype=np.int64)]))
-    g, r = _run(eng, wl, subset=sub)
+    g, r = _run(eng, wl, subset=sub, nslice=nslice)
     return _quartet_errors(g, r)
 
 
@@ -191,9 +194,10 @@ def test_config3_sampled(eng):
 
 
 def test_config4_sampled(eng):
-    """cfg 4 (ii|ii) K=5 per shell (625 primitive quartets): 1024-quartet launch, 3 quartets vs the oracle."""
+    """cfg 4 (ii|ii) K=5 per shell (625 primitive quartets): 1024-quartet launch, 2 quartets vs the oracle
+    (binary128: ~6 CPU-minutes per quartet, primitive loop spread over 16 threads)."""
     wl = inputs.config4()
-    errs, below = _sampled(eng, wl, 2, 104, extra=(0,))
+    errs, below = _sampled(eng, wl, 1, 104, extra=(0,), nslice=16)
     assert errs.max() <= TOL, errs.max()
 
 
@@ -203,7 +207,7 @@ def test_config5_classes_k3(eng, ci):
     wl = inputs.config5(ci, K=3)
     wl.bra_ij = wl.bra_ij[[0, 9, 63]]
     wl.ket_ij = wl.ket_ij[[5, 18, 60]]
-    g, r = _run(eng, wl)
+    g, r = _run(eng, wl, nslice=4)
     errs, below = _quartet_errors(g, r)
     assert errs.max() <= TOL, (wl.name, errs.max())
 
