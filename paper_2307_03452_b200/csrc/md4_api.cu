@@ -37,7 +37,7 @@ void free_shells(md4_ctx* c) {
 }
 
 void free_pair_storage(md4_pairs* p) {
-    cudaFree(p->d.H); cudaFree(p->d.scal); cudaFree(p->d.pairmax); cudaFree(p->d.ij);
+    cudaFree(p->d.Hb); cudaFree(p->d.Hk); cudaFree(p->d.scal); cudaFree(p->d.pairmax); cudaFree(p->d.ij);
     delete p;
 }
 
@@ -77,6 +77,14 @@ md4_status md4_create(md4_ctx** out, int cuda_device) {
     if (e == cudaSuccess) e = upload(&c->table_allocs, c->htab.tuv.data(), c->htab.tuv.size(), &d_tuv);
     if (e == cudaSuccess) e = upload(&c->table_allocs, c->htab.boys.data(), c->htab.boys.size(), &d_boys);
     c->tab.rtab = d_rtab; c->tab.tuv = d_tuv; c->tab.boys = d_boys;
+    for (int lp = 0; lp <= LPAIR && e == cudaSuccess; ++lp) {
+        uint32_t* dc = nullptr;
+        int* di = nullptr;
+        e = upload(&c->table_allocs, c->htab.colb[lp].data(), c->htab.colb[lp].size(), &dc);
+        c->tab.colb[lp] = dc;
+        if (e == cudaSuccess) { e = upload(&c->table_allocs, c->htab.colk[lp].data(), c->htab.colk[lp].size(), &dc); c->tab.colk[lp] = dc; }
+        if (e == cudaSuccess) { e = upload(&c->table_allocs, c->htab.b2k[lp].data(), c->htab.b2k[lp].size(), &di); c->tab.b2k[lp] = di; }
+    }
     for (int l = 0; l <= LMAX && e == cudaSuccess; ++l) {
         double* d = nullptr;
         e = upload(&c->table_allocs, c->htab.solid[l].data(), c->htab.solid[l].size(), &d);
@@ -170,8 +178,10 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
     d.nab = n_solid(d.li) * n_solid(d.lj);
     d.nrb = (d.nab + 7) / 8;
     d.nherm = n_hermite(d.lsum);
-    d.ncb = (d.nherm + 7) / 8;
-    d.hstride = (size_t)d.ncb * d.nrb * 64;
+    d.ncbb = (int)ctx->htab.colb[d.lsum].size() / 8;
+    d.ncbk = (int)ctx->htab.colk[d.lsum].size() / 8;
+    d.hstrideb = (size_t)d.ncbb * d.nrb * 64;
+    d.hstridek = (size_t)d.ncbk * d.nrb * 64;
     md4_pairs* pl = new (std::nothrow) md4_pairs();
     if (!pl) return fail(ctx, MD4_ENOMEM, "md4_build_pairs: out of host memory");
     pl->ctx = ctx;
@@ -179,7 +189,8 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
     if (npair > 0) {
         DeviceGuard g(ctx->device);
         const size_t nprim = (size_t)npair * d.Ki * d.Kj;
-        cudaError_t e = cudaMalloc((void**)&pl->d.H, nprim * d.hstride * sizeof(double));
+        cudaError_t e = cudaMalloc((void**)&pl->d.Hb, nprim * d.hstrideb * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.Hk, nprim * d.hstridek * sizeof(double));
         if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.scal, nprim * 8 * sizeof(double));
         if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.pairmax, (size_t)npair * sizeof(double));
         if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.ij, (size_t)npair * 2 * sizeof(int));
@@ -323,16 +334,25 @@ md4_status md4_debug_pair_h(md4_ctx* ctx, const md4_pairs* pairs, int ipair, int
     const int kk = d.Ki * d.Kj;
     if (ipair < 0 || ipair >= d.npair || iprim < 0 || iprim >= kk) return fail(ctx, MD4_EINVAL, "md4_debug_pair_h: index out of range");
     DeviceGuard g(ctx->device);
-    std::vector<double> blk(d.hstride);
+    std::vector<double> blk(d.hstrideb), blk2(d.hstridek);
     double s8[8], pm = 0.0;
     const size_t ip = (size_t)ipair * kk + iprim;
-    cudaError_t e = cudaMemcpy(blk.data(), d.H + ip * d.hstride, d.hstride * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaError_t e = cudaMemcpy(blk.data(), d.Hb + ip * d.hstrideb, d.hstrideb * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(blk2.data(), d.Hk + ip * d.hstridek, d.hstridek * sizeof(double), cudaMemcpyDeviceToHost);
     if (e == cudaSuccess) e = cudaMemcpy(s8, d.scal + ip * 8, sizeof(s8), cudaMemcpyDeviceToHost);
     if (e == cudaSuccess) e = cudaMemcpy(&pm, d.pairmax + ipair, sizeof(double), cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(ctx, "md4_debug_pair_h", e);
+    // out in graded Hermite order; the ket-role copy must hold the same numbers
+    const std::vector<int>& g2b = ctx->htab.g2b[d.lsum];
+    const std::vector<int>& b2k = ctx->htab.b2k[d.lsum];
     for (int r = 0; r < d.nab; ++r)
-        for (int c = 0; c < d.nherm; ++c)
-            out[(size_t)r * d.nherm + c] = blk[((size_t)(c >> 3) * d.nrb + (r >> 3)) * 64 + (r & 7) * 8 + (c & 7)];
+        for (int c = 0; c < d.nherm; ++c) {
+            const int cb = g2b[c], ck = b2k[cb];
+            const double vb = blk[((size_t)(cb >> 3) * d.nrb + (r >> 3)) * 64 + (r & 7) * 8 + (cb & 7)];
+            const double vk = blk2[((size_t)(ck >> 3) * d.nrb + (r >> 3)) * 64 + (r & 7) * 8 + (ck & 7)];
+            if (vb != vk && !(vb != vb && vk != vk)) return fail(ctx, MD4_ECUDA, "md4_debug_pair_h: bra-role and ket-role copies of H differ");
+            out[(size_t)r * d.nherm + c] = vb;
+        }
     scal[0] = s8[0]; scal[1] = s8[1]; scal[2] = s8[2]; scal[3] = s8[3]; scal[4] = s8[4] + pm;
     return MD4_OK;
 }

@@ -30,7 +30,7 @@ __device__ __forceinline__ double boys_one(const double* __restrict__ tab, int m
     return r;
 }
 
-// Builds R^{(0)}_{tuv}, t+u+v <= L, for one primitive quartet into Ra[t*S*S + u*S + v] (S = L+1).
+// Builds R^{(0)}_{tuv}, t+u+v <= L, for one primitive quartet into Ra[r_addr(t,u,v)] (md4_internal.h).
 // All threads of the CTA must call it.  Rc0/Rc1: two scratch arrays of n_hermite(L) doubles, sS: 32 doubles.
 // scale multiplies every value (K_ab K_cd relative to the pair maxima; 1 in the debug kernel).
 // Level l = 1..L computes [r]^(L-l) for all |r| <= l from level l-1 (one barrier per level, ping-pong
@@ -39,7 +39,7 @@ __device__ __forceinline__ double boys_one(const double* __restrict__ tab, int m
 __device__ __forceinline__ void hermite_r_block(double* Ra, double* Rc0, double* Rc1, double* sS,
                                                 const uint32_t* __restrict__ rtab,
                                                 const uint32_t* __restrict__ tuv,
-                                                const double* __restrict__ boys, int L, int S, double zp,
+                                                const double* __restrict__ boys, int L, double zp,
                                                 double Px, double Py, double Pz, double zq, double Qx, double Qy,
                                                 double Qz, double scale, int tid, int nthr) {
     const double X0 = Px - Qx, X1 = Py - Qy, X2 = Pz - Qz;
@@ -82,7 +82,7 @@ __device__ __forceinline__ void hermite_r_block(double* Ra, double* Rc0, double*
             }
             if (last) {
                 const uint32_t q = __ldg(tuv + e);
-                Ra[((q & 255) * S + ((q >> 8) & 255)) * S + ((q >> 16) & 255)] = val;
+                Ra[r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255)] = val;
             } else {
                 dst[e] = val;
             }
@@ -97,5 +97,30 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
+
+// ---- mbarrier / bulk-copy (TMA 1-D) primitives for the H_cd ring of the fused kernel -----------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n"
+        "W_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra D_%=;\n bra W_%=;\n"
+        "D_%=:\n}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared bulk copy; bytes % 16 == 0, both addresses 16-byte aligned; completion on bar
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 
 }  // namespace md4

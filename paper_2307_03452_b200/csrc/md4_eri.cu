@@ -1,16 +1,20 @@
 // md4_eri.cu -- the fused (ab|cd) kernel: S:8(a) steps a2-a9 in one launch.
 //
-// One CTA works on (one shell quartet) x (a group of 8-row blocks of the bra index ab); one warp owns
-// one 8-row block.  Per primitive quartet the CTA builds the Hermite Coulomb tensor R (Eq.10-13) in
-// shared memory; then every warp, independently,
+// One CTA works on (one shell quartet) x (a group of 8-row blocks of the bra index ab); one consumer warp
+// owns one 8-row block, one extra warp is the producer of the H_cd ring.  Per primitive quartet the CTA
+// builds the Hermite Coulomb tensor R (Eq.10-13) in shared memory; then every consumer warp, independently,
 //   GEMM1 (Eq.14/17):  T[8 x 8*NQT] = H_ab[8 rows, :] . G[:, q~ chunk],
-//          A fragments straight from global/L2 (each H_ab row block is used by exactly one warp),
+//          A fragments straight from global/L2, software-prefetched two k-blocks ahead (each H_ab row
+//          block is used by exactly one warp),
 //          B fragments gathered from shared memory: G[p~,q~] = (-1)^{|q~|} R[p~+q~] (Eq.8) read at
 //          address(p~) + address(q~) in the additive layout -- the 2-index integrals never exist in HBM
-//          (the paper writes them out), and not in shared memory either;
+//          (the paper writes them out), and not in shared memory either.  The column orders of
+//          H_ab / H_cd make this gather free of bank conflicts (md4_internal.h "Column orders");
 //   GEMM2 (Eq.15/18):  out[8 x Ncd] += T . H_cd[:, chunk]^T, A fragments = the C fragments of
 //          GEMM1 re-used in registers (the two DMMA k-steps of an 8-column block take the even and the
-//          odd columns, which is exactly what a lane holds), B fragments from global through L1.
+//          odd columns, which is exactly what a lane holds), B fragments from a shared-memory ring of
+//          H_cd column blocks that the producer warp fills with 1-D bulk copies (TMA) and all consumer
+//          warps of the CTA share (full/empty mbarriers per stage).
 // Both contractions run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> SASS DMMA.8x8x4; tcgen05 has
 // no f64 kind on sm_100a, S: facts table).  (ab|cd) accumulates in registers over all primitive
 // quartets (Listing 2.1) and is written once.
@@ -20,81 +24,101 @@ namespace md4 {
 
 namespace {
 
+constexpr int MAX_STAGES = 16;
+
 struct EriArgs {
     const double* Hb; const double* sb; const double* pmb; size_t hsb;
     const double* Hk; const double* sk; const double* pmk; size_t hsk;
     int Kb, Kk, nbra, nket;
-    int nab, ncd, nrb_ab, nrb_cd, ncb_p, ncb_q, nherm_p, nherm_q;
-    int L, S, wpc, ncta_per_q;
+    int nab, ncd, nrb_ab, nrb_cd, ncb_p, ncb_q;
+    int L, wpc, ncta_per_q, nst;
     long long nitems;
     const uint32_t* rtab; const uint32_t* tuv; const double* boys;
+    const uint32_t* colp; const uint32_t* colq;   // bra-order columns of the bra class, ket-order columns of the ket class
     double* out;
 };
 
-__host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
+__host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Shared memory: R in the additive layout | union { ping-pong scratch of the R recurrence, H_cd ring } |
+// seeds | gather offsets of the p~ and q~ columns | sign bits | mbarriers.
 struct SmemLayout {
-    size_t ra, rc0, rc1, ss, ap, aq, sg, total;
-    __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q) {
-        const int S = L + 1;
+    size_t ra, un, ss, ap, aq, sg, bars, total, stage_bytes, scratch_bytes;
+    __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst) {
         size_t o = 0;
-        ra = o; o += align16((size_t)S * S * S * 8);
-        rc0 = o; o += align16((size_t)n_hermite(L) * 8);
-        rc1 = o; o += align16((size_t)n_hermite(L) * 8);
+        ra = o; o += align_up((size_t)r_alloc(L) * 8, 128);
+        stage_bytes = (size_t)nrb_cd * 64 * 8;
+        scratch_bytes = align_up((size_t)n_hermite(L) * 8, 16) * 2;
+        const size_t ring = stage_bytes * nst;
+        un = o; o += align_up(ring > scratch_bytes ? ring : scratch_bytes, 128);
         ss = o; o += 32 * 8;
-        ap = o; o += align16((size_t)ncb_p * 8 * 4);
-        aq = o; o += align16((size_t)ncb_q * 8 * 4);
-        sg = o; o += align16((size_t)ncb_q * 4);
+        ap = o; o += align_up((size_t)ncb_p * 8 * 4, 16);
+        aq = o; o += align_up((size_t)ncb_q * 8 * 4, 16);
+        sg = o; o += align_up((size_t)ncb_q * 4, 16);
+        bars = o; o += 2 * MAX_STAGES * 8;
         total = o;
     }
 };
 
+__device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+
 template <int NT_CD, int NQT, int MAXW>
 __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
-    extern __shared__ __align__(16) unsigned char smem[];
-    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q);
+    extern __shared__ __align__(128) unsigned char smem[];
+    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
-    double* Rc0 = reinterpret_cast<double*>(smem + lay.rc0);
-    double* Rc1 = reinterpret_cast<double*>(smem + lay.rc1);
+    double* Rc0 = reinterpret_cast<double*>(smem + lay.un);
+    double* Rc1 = reinterpret_cast<double*>(smem + lay.un + lay.scratch_bytes / 2);
+    const double* ring = reinterpret_cast<const double*>(smem + lay.un);
     double* sS = reinterpret_cast<double*>(smem + lay.ss);
     int* ap = reinterpret_cast<int*>(smem + lay.ap);   // byte offset of p~ in Ra, per H_ab column
     int* aq = reinterpret_cast<int*>(smem + lay.aq);   // byte offset of q~ in Ra, per H_cd column
     unsigned* sg = reinterpret_cast<unsigned*>(smem + lay.sg);  // per q~ block: bit c set if |q~| odd
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + lay.bars);
+    uint64_t* empty = full + MAX_STAGES;
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
-    const int S = a.S, L = a.L;
+    const int L = a.L;
+    const int stage_doubles = a.nrb_cd * 64;
+    const uint32_t stage_bytes = (uint32_t)lay.stage_bytes;
 
-    // per-class gather tables (padding columns point at R_000: finite value times a zero of H)
+    // R array zeroed once: the recurrence always writes the same addresses, everything else (only ever
+    // read through padding columns, times a zero of H) stays 0
+    for (int i = tid; i < r_alloc(L); i += nthr) Ra[i] = 0.0;
     for (int c = tid; c < a.ncb_p * 8; c += nthr) {
-        int off = 0;
-        if (c < a.nherm_p) { const uint32_t q = __ldg(a.tuv + c); off = (((q & 255) * S + ((q >> 8) & 255)) * S + ((q >> 16) & 255)) * 8; }
-        ap[c] = off;
+        const uint32_t q = __ldg(a.colp + c);
+        ap[c] = r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255) * 8;
     }
     for (int c = tid; c < a.ncb_q * 8; c += nthr) {
-        int off = 0;
-        if (c < a.nherm_q) { const uint32_t q = __ldg(a.tuv + c); off = (((q & 255) * S + ((q >> 8) & 255)) * S + ((q >> 16) & 255)) * 8; }
-        aq[c] = off;
+        const uint32_t q = __ldg(a.colq + c);
+        aq[c] = r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255) * 8;
     }
     for (int b = tid; b < a.ncb_q; b += nthr) {
         unsigned m = 0;
         for (int c = 0; c < 8; ++c) {
-            const int col = b * 8 + c;
-            if (col < a.nherm_q) { const uint32_t q = __ldg(a.tuv + col); m |= (((q & 255) + ((q >> 8) & 255) + ((q >> 16) & 255)) & 1u) << c; }
+            const uint32_t q = __ldg(a.colq + b * 8 + c);
+            if (!(q & COL_PAD)) m |= (((q & 255) + ((q >> 8) & 255) + ((q >> 16) & 255)) & 1u) << c;
         }
         sg[b] = m;
+    }
+    if (tid == 0) {
+        for (int s = 0; s < a.nst; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)a.wpc); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
 
     const int nchunk = (a.ncb_q + NQT - 1) / NQT;
     const unsigned char* RaB = reinterpret_cast<const unsigned char*>(Ra);
     const int k4 = lane & 3, n8 = lane >> 2;
+    uint32_t cnt = 0;  // H_cd column blocks streamed through the ring so far (same count in every warp)
 
     for (long long item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const long long quartet = item / a.ncta_per_q;
         const int ms = (int)(item % a.ncta_per_q);
         const int ib = (int)(quartet / a.nket), jk = (int)(quartet % a.nket);
         const int mbk = ms * a.wpc + warp;       // 8-row block of ab owned by this warp
-        const bool active = (warp < a.wpc) && (mbk < a.nrb_ab);
+        const bool producer = (warp == a.wpc);
+        const bool active = !producer && (mbk < a.nrb_ab);
 
         double2 acc[NT_CD];
 #pragma unroll
@@ -103,14 +127,37 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
         for (int kq = 0; kq < a.Kk; ++kq) {
             const double* sq = a.sk + ((size_t)jk * a.Kk + kq) * 8;
             const double* Hq = a.Hk + ((size_t)jk * a.Kk + kq) * a.hsk;
-            for (int kp = 0; kp < a.Kb; ++kp) {
+            for (int kp = 0; kp < a.Kb; ++kp, cnt += (uint32_t)a.ncb_q) {
                 const double* sp = a.sb + ((size_t)ib * a.Kb + kp) * 8;
                 const double* Hp = a.Hb + ((size_t)ib * a.Kb + kp) * a.hsb;
-                __syncthreads();  // every warp is done with the previous R
-                hermite_r_block(Ra, Rc0, Rc1, sS, a.rtab, a.tuv, a.boys, L, S, __ldg(sp), __ldg(sp + 1),
+                __syncthreads();  // every warp is done with the previous R and with the ring (= R scratch)
+                hermite_r_block(Ra, Rc0, Rc1, sS, a.rtab, a.tuv, a.boys, L, __ldg(sp), __ldg(sp + 1),
                                 __ldg(sp + 2), __ldg(sp + 3), __ldg(sq), __ldg(sq + 1), __ldg(sq + 2),
                                 __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), tid, nthr);
-                if (!active) continue;
+                if (producer) {
+                    // ---- stream H_cd of this ket primitive through the ring, one column block per stage
+                    if (lane == 0) {
+                        fence_proxy_async();  // the scratch writes of the R recurrence precede the bulk copies
+                        for (int jq = 0; jq < a.ncb_q; ++jq) {
+                            const uint32_t c = cnt + (uint32_t)jq, s = c % (uint32_t)a.nst, ph = (c / (uint32_t)a.nst) & 1u;
+                            mbar_wait(empty + s, ph ^ 1u);
+                            mbar_expect_tx(full + s, stage_bytes);
+                            bulk_g2s(const_cast<double*>(ring) + (size_t)s * stage_doubles, Hq + (size_t)jq * stage_doubles,
+                                     stage_bytes, full + s);
+                        }
+                    }
+                    continue;
+                }
+                if (!active) {
+                    // a warp without rows still takes part in the ring protocol
+                    for (int jq = 0; jq < a.ncb_q; ++jq) {
+                        const uint32_t c = cnt + (uint32_t)jq, s = c % (uint32_t)a.nst, ph = (c / (uint32_t)a.nst) & 1u;
+                        mbar_wait(full + s, ph);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(empty + s);
+                    }
+                    continue;
+                }
                 const double* Ablk = Hp + (size_t)mbk * 64 + lane * 2;
                 const size_t astride = (size_t)a.nrb_ab * 64;
                 for (int ch = 0; ch < nchunk; ++ch) {
@@ -124,19 +171,20 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                         aqr[n] = (n < nq) ? aq[(j0 + n) * 8 + n8] : 0;
                     }
                     // ---- GEMM1: T = H_ab[8 rows] . G[:, chunk]
+                    double2 a0 = ldg2(Ablk);
+                    double2 a1 = a.ncb_p > 1 ? ldg2(Ablk + astride) : make_double2(0.0, 0.0);
 #pragma unroll 2
                     for (int jb = 0; jb < a.ncb_p; ++jb) {
-                        const double2 av = __ldg(reinterpret_cast<const double2*>(Ablk + (size_t)jb * astride));
+                        const double2 av = a0;
+                        a0 = a1;
+                        if (jb + 2 < a.ncb_p) a1 = ldg2(Ablk + (size_t)(jb + 2) * astride);
                         const int2 app = *reinterpret_cast<const int2*>(ap + jb * 8 + k4 * 2);
 #pragma unroll
-                        for (int n = 0; n < NQT; ++n) {
-                            if (n < nq) {
-                                const double b0 = *reinterpret_cast<const double*>(RaB + app.x + aqr[n]);
-                                const double b1 = *reinterpret_cast<const double*>(RaB + app.y + aqr[n]);
-                                dmma884(T[n].x, T[n].y, av.x, b0);
-                                dmma884(T[n].x, T[n].y, av.y, b1);
-                            }
-                        }
+                        for (int n = 0; n < NQT; ++n)
+                            if (n < nq) dmma884(T[n].x, T[n].y, av.x, *reinterpret_cast<const double*>(RaB + app.x + aqr[n]));
+#pragma unroll
+                        for (int n = 0; n < NQT; ++n)
+                            if (n < nq) dmma884(T[n].x, T[n].y, av.y, *reinterpret_cast<const double*>(RaB + app.y + aqr[n]));
                     }
                     // ---- sign of Eq.8 and GEMM2: acc += T . H_cd[:, chunk]^T
 #pragma unroll
@@ -145,15 +193,19 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                             const unsigned m = sg[j0 + n] >> (2 * k4);
                             const double tx = (m & 1u) ? -T[n].x : T[n].x;
                             const double ty = (m & 2u) ? -T[n].y : T[n].y;
-                            const double* Bblk = Hq + ((size_t)(j0 + n) * a.nrb_cd) * 64 + lane * 2;
+                            const uint32_t c = cnt + (uint32_t)(j0 + n), s = c % (uint32_t)a.nst, ph = (c / (uint32_t)a.nst) & 1u;
+                            mbar_wait(full + s, ph);
+                            const double* Bblk = ring + (size_t)s * stage_doubles + lane * 2;
 #pragma unroll
                             for (int nb = 0; nb < NT_CD; ++nb) {
                                 if (nb < a.nrb_cd) {
-                                    const double2 bv = __ldg(reinterpret_cast<const double2*>(Bblk + nb * 64));
+                                    const double2 bv = *reinterpret_cast<const double2*>(Bblk + nb * 64);
                                     dmma884(acc[nb].x, acc[nb].y, tx, bv.x);
                                     dmma884(acc[nb].x, acc[nb].y, ty, bv.y);
                                 }
                             }
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(empty + s);
                         }
                     }
                 }
@@ -178,8 +230,14 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
 }
 
 template <int NT_CD, int NQT, int MAXW>
-md4_status launch_one(md4_ctx* ctx, const EriArgs& a, cudaStream_t st) {
-    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q);
+md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
+    // ring depth: whatever shared memory is left after R, at least 2 stages, at most MAX_STAGES
+    int nst = 2;
+    for (int s = MAX_STAGES; s >= 2; --s)
+        if (SmemLayout(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, s).total <= (size_t)ctx->smem_optin) { nst = s; break; }
+    if (nst > a.ncb_q) nst = a.ncb_q < 2 ? 2 : a.ncb_q;
+    a.nst = nst;
+    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, nst);
     if (lay.total > (size_t)ctx->smem_optin) {
         ctx->err = "md4_compute: shared memory needed exceeds the device limit";
         return MD4_EUNSUPPORTED;
@@ -188,7 +246,7 @@ md4_status launch_one(md4_ctx* ctx, const EriArgs& a, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lay.total);
     if (e != cudaSuccess) { ctx->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return MD4_ECUDA; }
     long long grid = a.nitems < (long long)ctx->num_sms ? a.nitems : (long long)ctx->num_sms;
-    kern<<<(unsigned)grid, a.wpc * 32, lay.total, st>>>(a);
+    kern<<<(unsigned)grid, (a.wpc + 1) * 32, lay.total, st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) { ctx->err = std::string("eri_kernel launch: ") + cudaGetErrorString(e); return MD4_ECUDA; }
@@ -196,8 +254,8 @@ md4_status launch_one(md4_ctx* ctx, const EriArgs& a, cudaStream_t st) {
 }
 
 template <int NT_CD>
-md4_status launch_w(md4_ctx* ctx, const EriArgs& a, cudaStream_t st) {
-    if (a.wpc <= 8) return launch_one<NT_CD, 8, 8>(ctx, a, st);
+md4_status launch_w(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
+    if (a.wpc + 1 <= 9) return launch_one<NT_CD, 8, 9>(ctx, a, st);
     return launch_one<NT_CD, 8, 12>(ctx, a, st);
 }
 
@@ -206,17 +264,20 @@ md4_status launch_w(md4_ctx* ctx, const EriArgs& a, cudaStream_t st) {
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
                       cudaStream_t st) {
     EriArgs a;
-    a.Hb = bra.H; a.sb = bra.scal; a.pmb = bra.pairmax; a.hsb = bra.hstride;
-    a.Hk = ket.H; a.sk = ket.scal; a.pmk = ket.pairmax; a.hsk = ket.hstride;
+    a.Hb = bra.Hb; a.sb = bra.scal; a.pmb = bra.pairmax; a.hsb = bra.hstrideb;
+    a.Hk = ket.Hk; a.sk = ket.scal; a.pmk = ket.pairmax; a.hsk = ket.hstridek;
     a.Kb = bra.Ki * bra.Kj; a.Kk = ket.Ki * ket.Kj; a.nbra = bra.npair; a.nket = ket.npair;
     a.nab = bra.nab; a.ncd = ket.nab; a.nrb_ab = bra.nrb; a.nrb_cd = ket.nrb;
-    a.ncb_p = bra.ncb; a.ncb_q = ket.ncb; a.nherm_p = bra.nherm; a.nherm_q = ket.nherm;
-    a.L = bra.lsum + ket.lsum; a.S = a.L + 1;
-    // warps per CTA = 8-row blocks per CTA; a quartet is split over ncta_per_q CTAs
-    a.ncta_per_q = (a.nrb_ab + 11) / 12;
+    a.ncb_p = bra.ncbb; a.ncb_q = ket.ncbk;
+    a.L = bra.lsum + ket.lsum;
+    // consumer warps per CTA = 8-row blocks per CTA (<= 11, plus the producer warp); a quartet is split
+    // over ncta_per_q CTAs
+    a.ncta_per_q = (a.nrb_ab + 10) / 11;
     a.wpc = (a.nrb_ab + a.ncta_per_q - 1) / a.ncta_per_q;
     a.nitems = (long long)a.nbra * a.nket * a.ncta_per_q;
+    a.nst = 2;
     a.rtab = ctx->tab.rtab; a.tuv = ctx->tab.tuv; a.boys = ctx->tab.boys;
+    a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];
     a.out = d_out;
     const int nt = a.nrb_cd;
     if (nt <= 2) return launch_w<2>(ctx, a, st);
@@ -239,20 +300,24 @@ __global__ void debug_boys_kernel(const double* tab, int mmax, int n, const doub
     out[i] = boys_one(tab, i % (mmax + 1), T[i / (mmax + 1)]);
 }
 
+// out: dense [(L+1)^3] array, out[(t*(L+1)+u)*(L+1)+v] = R_{tuv} for t+u+v <= L, 0 elsewhere
 __global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const double* boys, int L, const double* pq,
                                double* out) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int S = L + 1;
     double* Ra = reinterpret_cast<double*>(smem);
-    double* Rc0 = Ra + S * S * S;
+    double* Rc0 = Ra + r_alloc(L);
     double* Rc1 = Rc0 + n_hermite(L);
     double* sS = Rc1 + n_hermite(L);
-    for (int i = threadIdx.x; i < S * S * S; i += blockDim.x) Ra[i] = 0.0;
+    for (int i = threadIdx.x; i < r_alloc(L); i += blockDim.x) Ra[i] = 0.0;
     __syncthreads();
-    hermite_r_block(Ra, Rc0, Rc1, sS, rtab, tuv, boys, L, S, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7],
+    hermite_r_block(Ra, Rc0, Rc1, sS, rtab, tuv, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7],
                     1.0, threadIdx.x, blockDim.x);
     __syncthreads();
-    for (int i = threadIdx.x; i < S * S * S; i += blockDim.x) out[i] = Ra[i];
+    for (int i = threadIdx.x; i < S * S * S; i += blockDim.x) {
+        const int t = i / (S * S), u = (i / S) % S, v = i % S;
+        out[i] = (t + u + v <= L) ? Ra[r_addr(t, u, v)] : 0.0;
+    }
 }
 }  // namespace
 
@@ -264,8 +329,7 @@ cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, 
 }
 
 cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out) {
-    const int S = L + 1;
-    const size_t sm = ((size_t)S * S * S + 2 * (size_t)n_hermite(L) + 32) * 8;
+    const size_t sm = ((size_t)r_alloc(L) + 2 * (size_t)n_hermite(L) + 32) * 8;
     cudaError_t e = cudaFuncSetAttribute(debug_r_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     debug_r_kernel<<<1, 256, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, L, d_pq, d_out);

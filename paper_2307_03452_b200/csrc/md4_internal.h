@@ -34,8 +34,25 @@ __host__ __device__ inline int herm_ord(int t, int u, int v) {
     return n * (n + 1) * (n + 2) / 6 + w * (w + 1) / 2 + (w - u);
 }
 
+// ---- additive layout of the Hermite Coulomb tensor in shared memory -------------------------------
+// R_{tuv} lives at r_addr(t,u,v) = t*RS2 + u*RS1 + v, so that address(p~ + q~) = address(p~) +
+// address(q~) and the 2-index integrals [p~|q~] = +-R_{p~+q~} (Eq.8) are a pure gather.  The
+// strides are the same for every class (the column order of H depends on them): RS1 > 24, RS2 > 24*RS1
+// keep the map injective on t+u+v <= 24, and their residues mod 16 (10 and 7) were chosen so that the
+// Hermite indices of every l_pair = 8..12 split almost evenly over the sixteen 8-byte bank pairs
+// (DESIGN.md "Conflict-free gather").
+constexpr int RS1 = 26;
+constexpr int RS2 = 631;
+__host__ __device__ inline int r_addr(int t, int u, int v) { return t * RS2 + u * RS1 + v; }
+__host__ __device__ inline int r_alloc(int L) { return L * RS2 + 32; }  // doubles; +32: padding columns read addresses 0..15 past the largest p~
+constexpr int LPAIR = 2 * LMAX;          // highest l_a + l_b of a shell pair
+constexpr uint32_t COL_PAD = 1u << 31;   // flag of a padding column in the column tables
+
 // Constant device tables, built once per context (md4_tables.cpp).
 struct DeviceTables {
+    const uint32_t* colb[LPAIR + 1];   // bra-role column order of H for l_pair: packed t | u<<8 | v<<16 | COL_PAD
+    const uint32_t* colk[LPAIR + 1];   // ket-role column order
+    const int* b2k[LPAIR + 1];         // bra column -> ket column of the same (t,u,v), -1 for padding
     const uint32_t* rtab;    // [NR_MAX] packed {idx0:12, idx1:12, C:5, axis:2} of Eq.13
     const uint32_t* tuv;     // [NR_MAX] packed t | u << 8 | v << 16 in graded order
     const double* boys;      // [BOYS_NODES * BOYS_STRIDE]
@@ -45,21 +62,32 @@ struct DeviceTables {
 
 struct HostTables {
     std::vector<uint32_t> rtab, tuv;
+    std::vector<uint32_t> colb[LPAIR + 1], colk[LPAIR + 1];   // sizes are multiples of 8
+    std::vector<int> b2k[LPAIR + 1], g2b[LPAIR + 1];          // g2b: graded ordinal -> bra column
     std::vector<double> boys;
     std::vector<double> solid[LMAX + 1], solid_lo[LMAX + 1];
 };
 void build_host_tables(HostTables& t);  // md4_tables.cpp
 
-// H matrices are stored in 8x8 blocks: element (row, col) of primitive pair ip lives at
-//   H[ip * hstride + ((col/8) * nrb + row/8) * 64 + (row%8) * 8 + col%8],
-// rows = solid-harmonic pair index ma*(2lj+1)+mb padded to nrb*8, cols = Hermite ordinal padded to
-// ncb*8, padding = 0.  One block is exactly the A fragment pair (bra role) or the B fragment pair
-// (ket role) of two DMMA.8x8x4 k-steps for a warp (lane*2 + {0,1}).
+// H matrices are stored in 8x8 blocks, once per role (two copies, same numbers, different column order):
+//   Hb (bra role, columns in colb order, ncbb blocks), Hk (ket role, colk order, ncbk blocks);
+// element (row, col) of primitive pair ip lives at
+//   H?[ip * hstride? + ((col/8) * nrb + row/8) * 64 + (row%8) * 8 + col%8],
+// rows = solid-harmonic pair index ma*(2lj+1)+mb padded to nrb*8, cols padded to whole blocks, padding = 0.
+// One block is exactly the A fragment pair (bra role: GEMM1) or the B fragment pair (ket role: GEMM2)
+// of two DMMA.8x8x4 k-steps for a warp (lane*2 + {0,1}).
+// Column orders (md4_tables.cpp build_orders): within a bra block the even columns and the odd columns
+// are the two k-steps, and the four p~ of a k-step sit in four consecutive 8-byte bank pairs {4g..4g+3}
+// of the additive R layout; within a ket block columns 0-3 and 4-7 (the two half warps of a B-fragment
+// gather) have bank pairs {c, c+4, c+8, c+12}.  The 16 lanes of a half warp then read 16 different bank
+// pairs: the gather of Eq.8 is free of shared-memory bank conflicts.
 struct PairListDev {
     int npair, li, lj, Ki, Kj;
-    int lsum, nab, nrb, nherm, ncb;
-    size_t hstride;      // doubles per primitive pair
-    double* H;           // [npair*Ki*Kj * hstride]
+    int lsum, nab, nrb, nherm;
+    int ncbb, ncbk;      // column blocks in bra / ket order
+    size_t hstrideb, hstridek;   // doubles per primitive pair
+    double* Hb;          // [npair*Ki*Kj * hstrideb]
+    double* Hk;          // [npair*Ki*Kj * hstridek]
     double* scal;        // [npair*Ki*Kj * 8]: zeta_p, Px, Py, Pz, lnK - pairmax, 0, 0, 0
     double* pairmax;     // [npair] max over primitives of ln K_ab
     int* ij;             // [npair*2]

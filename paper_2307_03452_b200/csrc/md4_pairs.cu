@@ -57,13 +57,15 @@ struct PairKernelArgs {
     const double* expo;
     const double* coef;
     const int* ij;
-    const uint32_t* tuv;
+    const uint32_t* colb;     // bra-role column order for this l_pair (md4_internal.h)
+    const int* b2k;           // bra column -> ket column
     const double *Ca, *CaLo;  // [(2li+1) * nc(li)] high / low parts
     const double *Cb, *CbLo;
-    double* H;
+    double* Hb;
+    double* Hk;
     double* scal;
-    int li, lj, Ki, Kj, nab, nrb, nherm, ncb;
-    size_t hstride;
+    int li, lj, Ki, Kj, nab, nrb, ncb;
+    size_t hstrideb, hstridek;
 };
 
 struct PairSmem {
@@ -163,8 +165,8 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
             const int pp = idx & 7, mb = (idx >> 3) % nsb, ac = (idx >> 3) / nsb;
             const int col = jb * 8 + pp;
             dd acc = make_double2(0.0, 0.0);
-            if (col < a.nherm) {
-                const uint32_t w = a.tuv[col];
+            const uint32_t w = a.colb[col];
+            if (!(w & COL_PAD)) {
                 const int t = w & 255, u = (w >> 8) & 255, v = (w >> 16) & 255;
                 const int ax = sm.ca[ac][0], ay = sm.ca[ac][1], az = li - ax - ay;
                 for (int bc = 0; bc < ncbt; ++bc) {
@@ -179,13 +181,18 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
         }
         __syncthreads();
         // half transform over a, contraction weight, blocked store
-        double* Hp = a.H + (size_t)ip * a.hstride + (size_t)jb * a.nrb * 64;
+        // (both role copies: the bra-order block here, the same number at its ket-order column there)
+        double* Hp = a.Hb + (size_t)ip * a.hstrideb + (size_t)jb * a.nrb * 64;
+        double* Hq = a.Hk + (size_t)ip * a.hstridek;
         for (int idx = tid; idx < a.nab * 8; idx += nthr) {
             const int pp = idx & 7, row = idx >> 3;
             const int ma = row / nsb, mb = row % nsb;
             dd acc = make_double2(0.0, 0.0);
             for (int ac = 0; ac < nca; ++ac) acc = dd_add(acc, dd_mul(sm.Ca[ma * nca + ac], sm.Y[(ac * nsb + mb) * 8 + pp]));
-            Hp[(row >> 3) * 64 + (row & 7) * 8 + pp] = wgt * acc.x + wgt * acc.y;
+            const double h = wgt * acc.x + wgt * acc.y;
+            Hp[(row >> 3) * 64 + (row & 7) * 8 + pp] = h;
+            const int ck = a.b2k[jb * 8 + pp];
+            if (ck >= 0) Hq[((size_t)(ck >> 3) * a.nrb + (row >> 3)) * 64 + (row & 7) * 8 + (ck & 7)] = h;
         }
         __syncthreads();
     }
@@ -205,16 +212,17 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
     if (pl.npair == 0) return cudaSuccess;
     const int kk = pl.Ki * pl.Kj;
     const size_t nprim = (size_t)pl.npair * kk;
-    cudaError_t e = cudaMemsetAsync(pl.H, 0, nprim * pl.hstride * sizeof(double), st);
+    cudaError_t e = cudaMemsetAsync(pl.Hb, 0, nprim * pl.hstrideb * sizeof(double), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pl.Hk, 0, nprim * pl.hstridek * sizeof(double), st);
     if (e != cudaSuccess) return e;
     PairKernelArgs a;
     a.centers = ctx->d_centers; a.off = ctx->d_off; a.expo = ctx->d_exp; a.coef = ctx->d_coef;
-    a.ij = pl.ij; a.tuv = ctx->tab.tuv;
+    a.ij = pl.ij; a.colb = ctx->tab.colb[pl.lsum]; a.b2k = ctx->tab.b2k[pl.lsum];
     a.Ca = ctx->tab.solid[pl.li]; a.CaLo = ctx->tab.solid_lo[pl.li];
     a.Cb = ctx->tab.solid[pl.lj]; a.CbLo = ctx->tab.solid_lo[pl.lj];
-    a.H = pl.H; a.scal = pl.scal;
+    a.Hb = pl.Hb; a.Hk = pl.Hk; a.scal = pl.scal;
     a.li = pl.li; a.lj = pl.lj; a.Ki = pl.Ki; a.Kj = pl.Kj;
-    a.nab = pl.nab; a.nrb = pl.nrb; a.nherm = pl.nherm; a.ncb = pl.ncb; a.hstride = pl.hstride;
+    a.nab = pl.nab; a.nrb = pl.nrb; a.ncb = pl.ncbb; a.hstrideb = pl.hstrideb; a.hstridek = pl.hstridek;
     const size_t nblk = nprim * PAIR_SPLIT;
     if (nblk > 2147483647ull) return cudaErrorInvalidValue;
     e = cudaFuncSetAttribute(pair_h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PairSmem));
