@@ -52,7 +52,7 @@ struct SmemLayout {
         const size_t ring = stage_bytes * nst;
         un = o; o += align_up(ring > scratch_bytes ? ring : scratch_bytes, 128);
         ss = o; o += 32 * 8;
-        ap = o; o += align_up((size_t)ncb_p * 8 * 4, 16);
+        ap = o; o += align_up((size_t)(ncb_p + 1) * 8 * 4, 16);   // one block of slack: the k-loop prefetches
         aq = o; o += align_up((size_t)ncb_q * 8 * 4, 16);
         sg = o; o += align_up((size_t)ncb_q * 4, 16);
         bars = o; o += 2 * MAX_STAGES * 8;
@@ -62,14 +62,102 @@ struct SmemLayout {
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 
-template <int NT_CD, int NQT, int MAXW>
+// Position in the H_cd ring; every warp of the CTA (producer, consumers with and without rows) steps
+// through the same sequence of column blocks, so the positions stay equal without communication.
+struct RingPos {
+    uint32_t s, ph;
+    __device__ __forceinline__ void advance(uint32_t nst) {
+        if (++s == nst) { s = 0; ph ^= 1u; }
+    }
+};
+
+// All shared-memory operands of the consumer loop are addressed by 32-bit shared addresses.
+struct ConsumerCtx {
+    const double* Ablk;    // this lane's A fragment pair of k-block 0 of the warp's 8-row block of H_ab
+    size_t astride;        // doubles between k-blocks of H_ab
+    uint32_t ra32;         // R in the additive layout
+    uint32_t ap32;         // ap + k4*2 (this lane's pair of p~ offsets in k-block 0)
+    uint32_t aq32;         // aq + n8 (this lane's q~ offset in q-block 0)
+    uint32_t sg32;         // sign bits per q-block
+    uint32_t ring32;       // ring + lane*16 bytes (this lane's B fragment pair of GEMM2)
+    uint32_t full32, empty32;
+    uint32_t stage_bytes, nst;
+    int ncb_p, nrb_cd, k4, lane;
+};
+
+// One chunk of NQ q~ blocks for one warp: T = H_ab[8 rows] . G[:, chunk] (GEMM1), then
+// acc += (sign . T) . H_cd[:, chunk]^T (GEMM2) against the ring.  PRED: q-blocks n >= nq are skipped
+// (general classes); otherwise nq == NQ.  EXACT: nrb_cd == NT_CD.
+template <int NQ, int NT_CD, bool EXACT, bool PRED>
+__device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const ConsumerCtx& c, int j0, int nq, RingPos& rp) {
+    double2 T[NQ];
+    uint32_t aqr[NQ];
+#pragma unroll
+    for (int n = 0; n < NQ; ++n) {
+        T[n] = make_double2(0.0, 0.0);
+        aqr[n] = c.ra32 + ((!PRED || n < nq) ? lds_u32(c.aq32 + (uint32_t)(j0 + n) * 32u) : 0u);
+    }
+    // ---- GEMM1: the B operand is G[p~,q~] = +-R[p~+q~] read at address(p~) + address(q~) (Eq.8)
+    double2 a0 = ldg2(c.Ablk);
+    double2 a1 = c.ncb_p > 1 ? ldg2(c.Ablk + c.astride) : make_double2(0.0, 0.0);
+    int2 apn = lds_v2s32(c.ap32);
+    for (int jb = 0; jb < c.ncb_p; ++jb) {
+        const double2 av = a0;
+        a0 = a1;
+        if (jb + 2 < c.ncb_p) a1 = ldg2(c.Ablk + (size_t)(jb + 2) * c.astride);
+        const int2 app = apn;
+        apn = lds_v2s32(c.ap32 + (uint32_t)(jb + 1) * 32u);   // the ap array has one block of slack
+        double b[NQ];
+#pragma unroll
+        for (int n = 0; n < NQ; ++n)
+            if (!PRED || n < nq) b[n] = lds_f64((uint32_t)app.x + aqr[n]);
+#pragma unroll
+        for (int n = 0; n < NQ; ++n)
+            if (!PRED || n < nq) dmma884(T[n].x, T[n].y, av.x, b[n]);
+#pragma unroll
+        for (int n = 0; n < NQ; ++n)
+            if (!PRED || n < nq) b[n] = lds_f64((uint32_t)app.y + aqr[n]);
+#pragma unroll
+        for (int n = 0; n < NQ; ++n)
+            if (!PRED || n < nq) dmma884(T[n].x, T[n].y, av.y, b[n]);
+    }
+    // ---- sign of Eq.8 and GEMM2: acc += T . H_cd[:, chunk]^T
+#pragma unroll
+    for (int n = 0; n < NQ; ++n) {
+        if (!PRED || n < nq) {
+            const uint32_t m = lds_u32(c.sg32 + (uint32_t)(j0 + n) * 4u) >> (2 * c.k4);
+            const double tx = (m & 1u) ? -T[n].x : T[n].x;
+            const double ty = (m & 2u) ? -T[n].y : T[n].y;
+            mbar_wait32(c.full32 + rp.s * 8u, rp.ph);
+            const uint32_t bb = c.ring32 + rp.s * c.stage_bytes;
+            constexpr int G = 4;   // B fragment pairs in flight
+#pragma unroll
+            for (int nb0 = 0; nb0 < NT_CD; nb0 += G) {
+                double2 bv[G];
+#pragma unroll
+                for (int g = 0; g < G; ++g)
+                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) bv[g] = lds_v2f64(bb + (uint32_t)(nb0 + g) * 512u);
+#pragma unroll
+                for (int g = 0; g < G; ++g)
+                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) {
+                        dmma884(acc[nb0 + g].x, acc[nb0 + g].y, tx, bv[g].x);
+                        dmma884(acc[nb0 + g].x, acc[nb0 + g].y, ty, bv[g].y);
+                    }
+            }
+            __syncwarp();
+            if (c.lane == 0) mbar_arrive32(c.empty32 + rp.s * 8u);
+            rp.advance(c.nst);
+        }
+    }
+}
+
+template <int NT_CD, int NQT, int MAXW, bool EXACT>
 __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
     double* Rc0 = reinterpret_cast<double*>(smem + lay.un);
     double* Rc1 = reinterpret_cast<double*>(smem + lay.un + lay.scratch_bytes / 2);
-    const double* ring = reinterpret_cast<const double*>(smem + lay.un);
     double* sS = reinterpret_cast<double*>(smem + lay.ss);
     int* ap = reinterpret_cast<int*>(smem + lay.ap);   // byte offset of p~ in Ra, per H_ab column
     int* aq = reinterpret_cast<int*>(smem + lay.aq);   // byte offset of q~ in Ra, per H_cd column
@@ -80,13 +168,12 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const int L = a.L;
     const int stage_doubles = a.nrb_cd * 64;
-    const uint32_t stage_bytes = (uint32_t)lay.stage_bytes;
 
     // R array zeroed once: the recurrence always writes the same addresses, everything else (only ever
     // read through padding columns, times a zero of H) stays 0
     for (int i = tid; i < r_alloc(L); i += nthr) Ra[i] = 0.0;
-    for (int c = tid; c < a.ncb_p * 8; c += nthr) {
-        const uint32_t q = __ldg(a.colp + c);
+    for (int c = tid; c < (a.ncb_p + 1) * 8; c += nthr) {
+        const uint32_t q = c < a.ncb_p * 8 ? __ldg(a.colp + c) : 0u;
         ap[c] = r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255) * 8;
     }
     for (int c = tid; c < a.ncb_q * 8; c += nthr) {
@@ -108,9 +195,23 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     __syncthreads();
 
     const int nchunk = (a.ncb_q + NQT - 1) / NQT;
-    const unsigned char* RaB = reinterpret_cast<const unsigned char*>(Ra);
-    const int k4 = lane & 3, n8 = lane >> 2;
-    uint32_t cnt = 0;  // H_cd column blocks streamed through the ring so far (same count in every warp)
+    ConsumerCtx cc;
+    cc.astride = (size_t)a.nrb_ab * 64;
+    cc.ra32 = smem_u32(Ra);
+    cc.k4 = lane & 3;
+    cc.lane = lane;
+    cc.ap32 = smem_u32(ap) + (uint32_t)cc.k4 * 8u;
+    cc.aq32 = smem_u32(aq) + (uint32_t)(lane >> 2) * 4u;
+    cc.sg32 = smem_u32(sg);
+    cc.ring32 = smem_u32(smem + lay.un) + (uint32_t)lane * 16u;
+    cc.full32 = smem_u32(full);
+    cc.empty32 = smem_u32(empty);
+    cc.stage_bytes = (uint32_t)lay.stage_bytes;
+    cc.nst = (uint32_t)a.nst;
+    cc.ncb_p = a.ncb_p;
+    cc.nrb_cd = a.nrb_cd;
+    const uint32_t ringbase32 = smem_u32(smem + lay.un);
+    RingPos rp{0u, 0u};  // same sequence in every warp
 
     for (long long item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const long long quartet = item / a.ncta_per_q;
@@ -127,7 +228,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
         for (int kq = 0; kq < a.Kk; ++kq) {
             const double* sq = a.sk + ((size_t)jk * a.Kk + kq) * 8;
             const double* Hq = a.Hk + ((size_t)jk * a.Kk + kq) * a.hsk;
-            for (int kp = 0; kp < a.Kb; ++kp, cnt += (uint32_t)a.ncb_q) {
+            for (int kp = 0; kp < a.Kb; ++kp) {
                 const double* sp = a.sb + ((size_t)ib * a.Kb + kp) * 8;
                 const double* Hp = a.Hb + ((size_t)ib * a.Kb + kp) * a.hsb;
                 __syncthreads();  // every warp is done with the previous R and with the ring (= R scratch)
@@ -139,75 +240,34 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                     if (lane == 0) {
                         fence_proxy_async();  // the scratch writes of the R recurrence precede the bulk copies
                         for (int jq = 0; jq < a.ncb_q; ++jq) {
-                            const uint32_t c = cnt + (uint32_t)jq, s = c % (uint32_t)a.nst, ph = (c / (uint32_t)a.nst) & 1u;
-                            mbar_wait(empty + s, ph ^ 1u);
-                            mbar_expect_tx(full + s, stage_bytes);
-                            bulk_g2s(const_cast<double*>(ring) + (size_t)s * stage_doubles, Hq + (size_t)jq * stage_doubles,
-                                     stage_bytes, full + s);
+                            mbar_wait32(cc.empty32 + rp.s * 8u, rp.ph ^ 1u);
+                            mbar_expect_tx32(cc.full32 + rp.s * 8u, cc.stage_bytes);
+                            bulk_g2s32(ringbase32 + rp.s * cc.stage_bytes, Hq + (size_t)jq * stage_doubles, cc.stage_bytes,
+                                       cc.full32 + rp.s * 8u);
+                            rp.advance(cc.nst);
                         }
                     }
+                    rp.s = __shfl_sync(0xffffffffu, rp.s, 0);
+                    rp.ph = __shfl_sync(0xffffffffu, rp.ph, 0);
                     continue;
                 }
                 if (!active) {
                     // a warp without rows still takes part in the ring protocol
                     for (int jq = 0; jq < a.ncb_q; ++jq) {
-                        const uint32_t c = cnt + (uint32_t)jq, s = c % (uint32_t)a.nst, ph = (c / (uint32_t)a.nst) & 1u;
-                        mbar_wait(full + s, ph);
+                        mbar_wait32(cc.full32 + rp.s * 8u, rp.ph);
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(empty + s);
+                        if (lane == 0) mbar_arrive32(cc.empty32 + rp.s * 8u);
+                        rp.advance(cc.nst);
                     }
                     continue;
                 }
-                const double* Ablk = Hp + (size_t)mbk * 64 + lane * 2;
-                const size_t astride = (size_t)a.nrb_ab * 64;
+                cc.Ablk = Hp + (size_t)mbk * 64 + lane * 2;
                 for (int ch = 0; ch < nchunk; ++ch) {
-                    const int j0 = (int)((long long)ch * a.ncb_q / nchunk);
-                    const int nq = (int)((long long)(ch + 1) * a.ncb_q / nchunk) - j0;
-                    double2 T[NQT];
-                    int aqr[NQT];
-#pragma unroll
-                    for (int n = 0; n < NQT; ++n) {
-                        T[n] = make_double2(0.0, 0.0);
-                        aqr[n] = (n < nq) ? aq[(j0 + n) * 8 + n8] : 0;
-                    }
-                    // ---- GEMM1: T = H_ab[8 rows] . G[:, chunk]
-                    double2 a0 = ldg2(Ablk);
-                    double2 a1 = a.ncb_p > 1 ? ldg2(Ablk + astride) : make_double2(0.0, 0.0);
-#pragma unroll 2
-                    for (int jb = 0; jb < a.ncb_p; ++jb) {
-                        const double2 av = a0;
-                        a0 = a1;
-                        if (jb + 2 < a.ncb_p) a1 = ldg2(Ablk + (size_t)(jb + 2) * astride);
-                        const int2 app = *reinterpret_cast<const int2*>(ap + jb * 8 + k4 * 2);
-#pragma unroll
-                        for (int n = 0; n < NQT; ++n)
-                            if (n < nq) dmma884(T[n].x, T[n].y, av.x, *reinterpret_cast<const double*>(RaB + app.x + aqr[n]));
-#pragma unroll
-                        for (int n = 0; n < NQT; ++n)
-                            if (n < nq) dmma884(T[n].x, T[n].y, av.y, *reinterpret_cast<const double*>(RaB + app.y + aqr[n]));
-                    }
-                    // ---- sign of Eq.8 and GEMM2: acc += T . H_cd[:, chunk]^T
-#pragma unroll
-                    for (int n = 0; n < NQT; ++n) {
-                        if (n < nq) {
-                            const unsigned m = sg[j0 + n] >> (2 * k4);
-                            const double tx = (m & 1u) ? -T[n].x : T[n].x;
-                            const double ty = (m & 2u) ? -T[n].y : T[n].y;
-                            const uint32_t c = cnt + (uint32_t)(j0 + n), s = c % (uint32_t)a.nst, ph = (c / (uint32_t)a.nst) & 1u;
-                            mbar_wait(full + s, ph);
-                            const double* Bblk = ring + (size_t)s * stage_doubles + lane * 2;
-#pragma unroll
-                            for (int nb = 0; nb < NT_CD; ++nb) {
-                                if (nb < a.nrb_cd) {
-                                    const double2 bv = *reinterpret_cast<const double2*>(Bblk + nb * 64);
-                                    dmma884(acc[nb].x, acc[nb].y, tx, bv.x);
-                                    dmma884(acc[nb].x, acc[nb].y, ty, bv.y);
-                                }
-                            }
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(empty + s);
-                        }
-                    }
+                    const int j0 = ch * a.ncb_q / nchunk;
+                    const int nq = (ch + 1) * a.ncb_q / nchunk - j0;
+                    if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
+                    else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
+                    else consume_chunk<NQT - 2, NT_CD, EXACT, true>(acc, cc, j0, nq, rp);
                 }
             }
         }
@@ -215,12 +275,12 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
         // results near the bottom of the FP64 range are still correctly rounded
         if (active) {
             const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
-            const int row = mbk * 8 + n8;
+            const int row = mbk * 8 + (lane >> 2);
             if (row < a.nab) {
                 double* o = a.out + (size_t)quartet * a.nab * a.ncd + (size_t)row * a.ncd;
 #pragma unroll
                 for (int nb = 0; nb < NT_CD; ++nb) {
-                    const int col = nb * 8 + 2 * k4;
+                    const int col = nb * 8 + 2 * cc.k4;
                     if (col < a.ncd) o[col] = (acc[nb].x * f) * f;
                     if (col + 1 < a.ncd) o[col + 1] = (acc[nb].y * f) * f;
                 }
@@ -229,7 +289,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     }
 }
 
-template <int NT_CD, int NQT, int MAXW>
+template <int NT_CD, int NQT, int MAXW, bool EXACT>
 md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
     // ring depth: whatever shared memory is left after R, at least 2 stages, at most MAX_STAGES
     int nst = 2;
@@ -242,7 +302,7 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
         ctx->err = "md4_compute: shared memory needed exceeds the device limit";
         return MD4_EUNSUPPORTED;
     }
-    auto kern = eri_kernel<NT_CD, NQT, MAXW>;
+    auto kern = eri_kernel<NT_CD, NQT, MAXW, EXACT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lay.total);
     if (e != cudaSuccess) { ctx->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return MD4_ECUDA; }
     long long grid = a.nitems < (long long)ctx->num_sms ? a.nitems : (long long)ctx->num_sms;
@@ -253,10 +313,10 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
     return MD4_OK;
 }
 
-template <int NT_CD>
+template <int NT_CD, bool EXACT>
 md4_status launch_w(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
-    if (a.wpc + 1 <= 9) return launch_one<NT_CD, 8, 9>(ctx, a, st);
-    return launch_one<NT_CD, 8, 12>(ctx, a, st);
+    if (a.wpc + 1 <= 9) return launch_one<NT_CD, 8, 9, EXACT>(ctx, a, st);
+    return launch_one<NT_CD, 8, 12, EXACT>(ctx, a, st);
 }
 
 }  // namespace
@@ -280,14 +340,18 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];
     a.out = d_out;
     const int nt = a.nrb_cd;
-    if (nt <= 2) return launch_w<2>(ctx, a, st);
-    if (nt <= 4) return launch_w<4>(ctx, a, st);
-    if (nt <= 7) return launch_w<7>(ctx, a, st);
-    if (nt <= 11) return launch_w<11>(ctx, a, st);
-    if (nt <= 13) return launch_w<13>(ctx, a, st);
-    if (nt <= 16) return launch_w<16>(ctx, a, st);
-    if (nt <= 18) return launch_w<18>(ctx, a, st);
-    if (nt <= 22) return launch_w<22>(ctx, a, st);
+    // exact instantiations for the ket classes of l >= 4 shells (N_cd = 81, 99, 117, 121, 143, 169); the
+    // others (no product of two odd numbers <= 13 falls in 14, 17, 19-21 row blocks) run predicated
+    if (nt == 11) return launch_w<11, true>(ctx, a, st);
+    if (nt == 13) return launch_w<13, true>(ctx, a, st);
+    if (nt == 15) return launch_w<15, true>(ctx, a, st);
+    if (nt == 16) return launch_w<16, true>(ctx, a, st);
+    if (nt == 18) return launch_w<18, true>(ctx, a, st);
+    if (nt == 22) return launch_w<22, true>(ctx, a, st);
+    if (nt <= 2) return launch_w<2, false>(ctx, a, st);
+    if (nt <= 4) return launch_w<4, false>(ctx, a, st);
+    if (nt <= 7) return launch_w<7, false>(ctx, a, st);
+    if (nt <= 12) return launch_w<12, false>(ctx, a, st);
     ctx->err = "md4_compute: ket class too large";
     return MD4_EUNSUPPORTED;
 }
