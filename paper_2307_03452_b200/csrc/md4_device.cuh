@@ -32,13 +32,24 @@ __device__ __forceinline__ double boys_one(const double* __restrict__ tab, int m
 
 // Builds R^{(0)}_{tuv}, t+u+v <= L, for one primitive quartet into Ra[r_addr(t,u,v)] (md4_internal.h).
 // All threads of the CTA must call it.  Rc0/Rc1: two scratch arrays of n_hermite(L) doubles, sS: 32 doubles.
+// srt / sad: shared-memory copies of the Eq.13 table and of the additive address of every graded ordinal
+// (r_tables_to_smem below) -- the table is m-independent, so it is read from shared memory at
+// every level instead of from global memory.
 // scale multiplies every value (K_ab K_cd relative to the pair maxima; 1 in the debug kernel).
 // Level l = 1..L computes [r]^(L-l) for all |r| <= l from level l-1 (one barrier per level, ping-pong
 // buffers instead of the paper's in-place array with two barriers; the last level scatters into the
 // additive layout so that address(p~ + q~) = address(p~) + address(q~), Eq.8 as a pure gather).
+__device__ __forceinline__ void r_tables_to_smem(uint32_t* srt, uint16_t* sad, const uint32_t* __restrict__ rtab,
+                                                 const uint32_t* __restrict__ tuv, int L, int tid, int nthr) {
+    for (int e = tid; e < n_hermite(L); e += nthr) {
+        srt[e] = __ldg(rtab + e);
+        const uint32_t q = __ldg(tuv + e);
+        sad[e] = (uint16_t)r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255);
+    }
+}
+
 __device__ __forceinline__ void hermite_r_block(double* Ra, double* Rc0, double* Rc1, double* sS,
-                                                const uint32_t* __restrict__ rtab,
-                                                const uint32_t* __restrict__ tuv,
+                                                const uint32_t* srt, const uint16_t* sad,
                                                 const double* __restrict__ boys, int L, double zp,
                                                 double Px, double Py, double Pz, double zq, double Qx, double Qy,
                                                 double Qz, double scale, int tid, int nthr) {
@@ -67,24 +78,31 @@ __device__ __forceinline__ void hermite_r_block(double* Ra, double* Rc0, double*
     double* dst = Rc1;
     if (tid == 0) src[0] = sS[L];
     __syncthreads();
+    constexpr int B = 4;  // independent elements in flight per thread
     for (int l = 1; l <= L; ++l) {
         const int n = n_hermite(l);
         const bool last = (l == L);
-        for (int e = tid; e < n; e += nthr) {
-            double val;
-            if (e == 0) {
-                val = sS[L - l];
-            } else {
-                const uint32_t w = __ldg(rtab + e);
-                const int i0 = w & 4095, i1 = (w >> 12) & 4095, C = (w >> 24) & 31, ax = (w >> 29) & 3;
-                const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
-                val = fma((double)C, src[i0], x * src[i1]);
+        for (int e0 = tid; e0 < n; e0 += B * nthr) {
+            double val[B];
+#pragma unroll
+            for (int k = 0; k < B; ++k) {
+                const int e = e0 + k * nthr;
+                if (e == 0) {
+                    val[k] = sS[L - l];
+                } else if (e < n) {
+                    const uint32_t w = srt[e];
+                    const int i0 = w & 4095, i1 = (w >> 12) & 4095, C = (w >> 24) & 31, ax = (w >> 29) & 3;
+                    const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
+                    val[k] = fma((double)C, src[i0], x * src[i1]);
+                }
             }
-            if (last) {
-                const uint32_t q = __ldg(tuv + e);
-                Ra[r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255)] = val;
-            } else {
-                dst[e] = val;
+#pragma unroll
+            for (int k = 0; k < B; ++k) {
+                const int e = e0 + k * nthr;
+                if (e < n) {
+                    if (last) Ra[sad[e]] = val[k];
+                    else dst[e] = val[k];
+                }
             }
         }
         __syncthreads();

@@ -18,6 +18,9 @@
 // Both contractions run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> SASS DMMA.8x8x4; tcgen05 has
 // no f64 kind on sm_100a, S: facts table).  (ab|cd) accumulates in registers over all primitive
 // quartets (Listing 2.1) and is written once.
+#ifdef MD4_PHASE_TIMING
+namespace md4 { __device__ unsigned long long g_phase[8]; }
+#endif
 #include "md4_device.cuh"
 
 namespace md4 {
@@ -43,7 +46,7 @@ __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a -
 // Shared memory: R in the additive layout | union { ping-pong scratch of the R recurrence, H_cd ring } |
 // seeds | gather offsets of the p~ and q~ columns | sign bits | mbarriers.
 struct SmemLayout {
-    size_t ra, un, ss, ap, aq, sg, bars, total, stage_bytes, scratch_bytes;
+    size_t ra, un, ss, ap, aq, sg, rt, ad, bars, total, stage_bytes, scratch_bytes;
     __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst) {
         size_t o = 0;
         ra = o; o += align_up((size_t)r_alloc(L) * 8, 128);
@@ -55,6 +58,8 @@ struct SmemLayout {
         ap = o; o += align_up((size_t)(ncb_p + 1) * 8 * 4, 16);   // one block of slack: the k-loop prefetches
         aq = o; o += align_up((size_t)ncb_q * 8 * 4, 16);
         sg = o; o += align_up((size_t)ncb_q * 4, 16);
+        rt = o; o += align_up((size_t)n_hermite(L) * 4, 16);   // Eq.13 table
+        ad = o; o += align_up((size_t)n_hermite(L) * 2, 16);   // additive address per graded ordinal
         bars = o; o += 2 * MAX_STAGES * 8;
         total = o;
     }
@@ -64,6 +69,15 @@ __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterp
 
 // Position in the H_cd ring; every warp of the CTA (producer, consumers with and without rows) steps
 // through the same sequence of column blocks, so the positions stay equal without communication.
+#ifdef MD4_PHASE_TIMING
+// developer instrumentation (not compiled into the product): cycles per phase summed over consumer warps
+#define PT_DECL unsigned long long pt_t = clock64();
+#define PT_MARK(i) { const unsigned long long pt_n = clock64(); if (threadIdx.x % 32 == 0) atomicAdd(&g_phase[i], pt_n - pt_t); pt_t = pt_n; }
+#else
+#define PT_DECL
+#define PT_MARK(i)
+#endif
+
 struct RingPos {
     uint32_t s, ph;
     __device__ __forceinline__ void advance(uint32_t nst) {
@@ -92,6 +106,7 @@ template <int NQ, int NT_CD, bool EXACT, bool PRED>
 __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const ConsumerCtx& c, int j0, int nq, RingPos& rp) {
     double2 T[NQ];
     uint32_t aqr[NQ];
+    PT_DECL
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
         T[n] = make_double2(0.0, 0.0);
@@ -121,6 +136,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
         for (int n = 0; n < NQ; ++n)
             if (!PRED || n < nq) dmma884(T[n].x, T[n].y, av.y, b[n]);
     }
+    PT_MARK(1)
     // ---- sign of Eq.8 and GEMM2: acc += T . H_cd[:, chunk]^T
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
@@ -128,7 +144,9 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
             const uint32_t m = lds_u32(c.sg32 + (uint32_t)(j0 + n) * 4u) >> (2 * c.k4);
             const double tx = (m & 1u) ? -T[n].x : T[n].x;
             const double ty = (m & 2u) ? -T[n].y : T[n].y;
+            PT_MARK(2)
             mbar_wait32(c.full32 + rp.s * 8u, rp.ph);
+            PT_MARK(3)
             const uint32_t bb = c.ring32 + rp.s * c.stage_bytes;
             constexpr int G = 4;   // B fragment pairs in flight
 #pragma unroll
@@ -139,16 +157,17 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
                     if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) bv[g] = lds_v2f64(bb + (uint32_t)(nb0 + g) * 512u);
 #pragma unroll
                 for (int g = 0; g < G; ++g)
-                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) {
-                        dmma884(acc[nb0 + g].x, acc[nb0 + g].y, tx, bv[g].x);
-                        dmma884(acc[nb0 + g].x, acc[nb0 + g].y, ty, bv[g].y);
-                    }
+                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) dmma884(acc[nb0 + g].x, acc[nb0 + g].y, tx, bv[g].x);
+#pragma unroll
+                for (int g = 0; g < G; ++g)
+                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) dmma884(acc[nb0 + g].x, acc[nb0 + g].y, ty, bv[g].y);
             }
             __syncwarp();
             if (c.lane == 0) mbar_arrive32(c.empty32 + rp.s * 8u);
             rp.advance(c.nst);
         }
     }
+    PT_MARK(2)
 }
 
 template <int NT_CD, int NQT, int MAXW, bool EXACT>
@@ -162,6 +181,8 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     int* ap = reinterpret_cast<int*>(smem + lay.ap);   // byte offset of p~ in Ra, per H_ab column
     int* aq = reinterpret_cast<int*>(smem + lay.aq);   // byte offset of q~ in Ra, per H_cd column
     unsigned* sg = reinterpret_cast<unsigned*>(smem + lay.sg);  // per q~ block: bit c set if |q~| odd
+    uint32_t* srt = reinterpret_cast<uint32_t*>(smem + lay.rt);
+    uint16_t* sad = reinterpret_cast<uint16_t*>(smem + lay.ad);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + lay.bars);
     uint64_t* empty = full + MAX_STAGES;
 
@@ -172,6 +193,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     // R array zeroed once: the recurrence always writes the same addresses, everything else (only ever
     // read through padding columns, times a zero of H) stays 0
     for (int i = tid; i < r_alloc(L); i += nthr) Ra[i] = 0.0;
+    r_tables_to_smem(srt, sad, a.rtab, a.tuv, L, tid, nthr);
     for (int c = tid; c < (a.ncb_p + 1) * 8; c += nthr) {
         const uint32_t q = c < a.ncb_p * 8 ? __ldg(a.colp + c) : 0u;
         ap[c] = r_addr(q & 255, (q >> 8) & 255, (q >> 16) & 255) * 8;
@@ -231,8 +253,10 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
             for (int kp = 0; kp < a.Kb; ++kp) {
                 const double* sp = a.sb + ((size_t)ib * a.Kb + kp) * 8;
                 const double* Hp = a.Hb + ((size_t)ib * a.Kb + kp) * a.hsb;
+                PT_DECL
                 __syncthreads();  // every warp is done with the previous R and with the ring (= R scratch)
-                hermite_r_block(Ra, Rc0, Rc1, sS, a.rtab, a.tuv, a.boys, L, __ldg(sp), __ldg(sp + 1),
+                PT_MARK(4)
+                hermite_r_block(Ra, Rc0, Rc1, sS, srt, sad, a.boys, L, __ldg(sp), __ldg(sp + 1),
                                 __ldg(sp + 2), __ldg(sp + 3), __ldg(sq), __ldg(sq + 1), __ldg(sq + 2),
                                 __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), tid, nthr);
                 if (producer) {
@@ -273,6 +297,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
         }
         // ---- epilogue: common factor K_ab K_cd of the pair maxima, applied in two halves so that
         // results near the bottom of the FP64 range are still correctly rounded
+        PT_DECL
         if (active) {
             const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
             const int row = mbk * 8 + (lane >> 2);
@@ -286,6 +311,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                 }
             }
         }
+        PT_MARK(5)
     }
 }
 
@@ -356,6 +382,14 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     return MD4_EUNSUPPORTED;
 }
 
+#ifdef MD4_PHASE_TIMING
+extern "C" void md4_debug_phase_cycles(unsigned long long* out8, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out8, g_phase, sizeof(g_phase));
+    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_phase, z, sizeof(z)); }
+}
+#endif
+
 // ---- stage-level debug kernels ---------------------------------------------------------------------
 namespace {
 __global__ void debug_boys_kernel(const double* tab, int mmax, int n, const double* T, double* out) {
@@ -373,9 +407,12 @@ __global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const 
     double* Rc0 = Ra + r_alloc(L);
     double* Rc1 = Rc0 + n_hermite(L);
     double* sS = Rc1 + n_hermite(L);
+    uint32_t* srt = reinterpret_cast<uint32_t*>(sS + 32);
+    uint16_t* sad = reinterpret_cast<uint16_t*>(srt + n_hermite(L));
     for (int i = threadIdx.x; i < r_alloc(L); i += blockDim.x) Ra[i] = 0.0;
+    r_tables_to_smem(srt, sad, rtab, tuv, L, threadIdx.x, blockDim.x);
     __syncthreads();
-    hermite_r_block(Ra, Rc0, Rc1, sS, rtab, tuv, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7],
+    hermite_r_block(Ra, Rc0, Rc1, sS, srt, sad, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7],
                     1.0, threadIdx.x, blockDim.x);
     __syncthreads();
     for (int i = threadIdx.x; i < S * S * S; i += blockDim.x) {
@@ -393,7 +430,7 @@ cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, 
 }
 
 cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out) {
-    const size_t sm = ((size_t)r_alloc(L) + 2 * (size_t)n_hermite(L) + 32) * 8;
+    const size_t sm = ((size_t)r_alloc(L) + 2 * (size_t)n_hermite(L) + 32) * 8 + (size_t)n_hermite(L) * 6 + 16;
     cudaError_t e = cudaFuncSetAttribute(debug_r_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     debug_r_kernel<<<1, 256, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, L, d_pq, d_out);
