@@ -175,6 +175,27 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------------- GPU arm
+def reduce_max(x: float, world: int, device: str) -> float:
+    """Max over ranks of a host scalar (the only collective of the bench: quartets are independent, S:8(e))."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world: int, quartets_per_rank: int, ms_per_step: float) -> float:
+    """Whole-job quartets/s: every rank processes its own batch of quartets_per_rank in the max-over-ranks time."""
+    return world * quartets_per_rank / (ms_per_step * 1e-3)
+
+
+# ncu --set full capture of the dominant kernel (profiles/r1_eri_kernel_ncu.md): dram read + write bytes per launch
+NCU_TRAFFIC_BYTES = {"cfg3": 12.77e9}
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -206,8 +227,14 @@ def run_gpu(args):
     out = torch.empty(out_doubles, dtype=torch.float64, device=f"cuda:{local}")
 
     kern_ev = []
+    prev = []
 
     def step(timed: bool):
+        # the lists of the step before are released first (md4_free_pairs waits for the work that reads them and
+        # hands their buffers to the next md4_build_pairs): the loop a user of the library would write
+        while prev:
+            b, k = prev.pop()
+            b.free(); k.free()
         bra = eng.build_pairs(wl.bra_ij)
         ket = eng.build_pairs(wl.ket_ij)
         if timed:
@@ -217,16 +244,12 @@ def run_gpu(args):
         if timed:
             e1.record(stream)
             kern_ev.append((e0, e1))
-        return bra, ket
-
-    def free(lists):
-        for b, k in lists:
-            b.free(); k.free()
+        prev.append((bra, ket))
 
     # ---- device-resident arm: W warm-up steps, then exactly K timed steps
-    live = [step(False) for _ in range(args.warmup)]
+    for _ in range(args.warmup):
+        step(False)
     barrier()
-    free(live)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -234,20 +257,19 @@ def run_gpu(args):
     barrier()
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0.record(stream)
-    live = [step(True) for _ in range(args.steps)]
+    for _ in range(args.steps):
+        step(True)
     t1.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else {}
     n_launch = eng.launch_count() - n_launch0
-    free(live)
-    ms_total = t0.elapsed_time(t1)
+    while prev:
+        b, k = prev.pop()
+        b.free(); k.free()
+    ms_total = reduce_max(t0.elapsed_time(t1), world, f"cuda:{local}")
     kern_ms = [a.elapsed_time(b) for a, b in kern_ev]
-    tt = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_total = float(tt.item())
     ms_step = ms_total / args.steps
-    value = world * nq / (ms_step * 1e-3)
+    value = whole_job_rate(world, nq, ms_step)
 
     # ---- end-to-end arm through HOST buffers (same K steps; H2D of shells + pair lists, D2H of all integrals)
     host = torch.empty(out_doubles, dtype=torch.float64, pin_memory=True)
@@ -269,11 +291,8 @@ def run_gpu(args):
     for _ in range(args.steps):
         e2e_step()
     barrier()
-    e2e_s = time.perf_counter() - w0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * nq * args.steps / float(te.item())
+    e2e_s = reduce_max(time.perf_counter() - w0, world, f"cuda:{local}")
+    e2e_value = whole_job_rate(world, nq, 1e3 * e2e_s / args.steps)
 
     if rank == 0:
         peak, peak_how = fp64_peak_tflops()
@@ -289,7 +308,9 @@ def run_gpu(args):
             "tflops": value * flops_q / 1e12, "fp64_peak_frac": value * flops_q / 1e12 / (peak * world),
             "flops_per_quartet": flops_q,
             "roofline": {"bound": "tensor", "kernel": "md4::eri_kernel (FP64 DMMA.8x8x4)", "achieved": achieved,
-                         "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                         "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                         "traffic_unit": "bytes per launch (dram read+write, profiles/r1_eri_kernel_ncu.md)",
+                         "algorithmic_bytes": out_doubles * 8,
                          "peak_source": peak_how, "kernel_ms": k_ms},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(n_launch), "clocks": clocks,

@@ -36,8 +36,53 @@ void free_shells(md4_ctx* c) {
     c->nshell = 0; c->nprim = 0; c->h_l.clear(); c->h_off.clear();
 }
 
-void free_pair_storage(md4_pairs* p) {
-    cudaFree(p->d.Hb); cudaFree(p->d.Hk); cudaFree(p->d.scal); cudaFree(p->d.pairmax); cudaFree(p->d.ij);
+// ---- pool of H buffers ------------------------------------------------------------------------------
+constexpr size_t POOL_MIN_BYTES = (size_t)1 << 20;    // smaller blocks go straight to cudaMalloc/cudaFree
+constexpr size_t POOL_MAX_BYTES = (size_t)16 << 30;   // bytes kept idle at most
+
+cudaError_t pool_alloc(md4_ctx* c, size_t bytes, double** out) {
+    *out = nullptr;
+    if (bytes >= POOL_MIN_BYTES) {
+        auto it = c->pool.lower_bound(bytes);
+        if (it != c->pool.end() && it->first <= bytes + bytes / 4) {
+            *out = static_cast<double*>(it->second);
+            c->pool_bytes -= it->first;
+            c->pool.erase(it);
+            return cudaSuccess;
+        }
+    }
+    cudaError_t e = cudaMalloc((void**)out, bytes ? bytes : 8);
+    if (e == cudaErrorMemoryAllocation && !c->pool.empty()) {
+        (void)cudaGetLastError();
+        for (auto& kv : c->pool) cudaFree(kv.second);
+        c->pool.clear(); c->pool_bytes = 0;
+        e = cudaMalloc((void**)out, bytes ? bytes : 8);
+    }
+    return e;
+}
+
+void pool_free(md4_ctx* c, void* p, size_t bytes) {
+    if (!p) return;
+    if (c && bytes >= POOL_MIN_BYTES && c->pool_bytes + bytes <= POOL_MAX_BYTES) {
+        c->pool.emplace(bytes, p);
+        c->pool_bytes += bytes;
+    } else {
+        cudaFree(p);
+    }
+}
+
+void pool_release(md4_ctx* c) {
+    for (auto& kv : c->pool) cudaFree(kv.second);
+    c->pool.clear(); c->pool_bytes = 0;
+}
+
+// to_pool: the list's work on the device is known to be complete, its H buffers may be reused
+void free_pair_storage(md4_pairs* p, bool to_pool) {
+    const size_t nprim = (size_t)p->d.npair * p->d.Ki * p->d.Kj;
+    md4_ctx* c = to_pool ? p->ctx : nullptr;
+    pool_free(c, p->d.Hb, nprim * p->d.hstrideb * sizeof(double));
+    pool_free(c, p->d.Hk, nprim * p->d.hstridek * sizeof(double));
+    cudaFree(p->d.scal); cudaFree(p->d.pairmax); cudaFree(p->d.ij);
     delete p;
 }
 
@@ -107,8 +152,10 @@ md4_status md4_create(md4_ctx** out, int cuda_device) {
 void md4_destroy(md4_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard g(ctx->device);
-    for (md4_pairs* p : ctx->lists) free_pair_storage(p);
+    cudaDeviceSynchronize();
+    for (md4_pairs* p : ctx->lists) free_pair_storage(p, false);
     ctx->lists.clear();
+    pool_release(ctx);
     free_shells(ctx);
     cudaFree(ctx->d_scratch);
     for (void* p : ctx->table_allocs) cudaFree(p);
@@ -189,15 +236,15 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
     if (npair > 0) {
         DeviceGuard g(ctx->device);
         const size_t nprim = (size_t)npair * d.Ki * d.Kj;
-        cudaError_t e = cudaMalloc((void**)&pl->d.Hb, nprim * d.hstrideb * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.Hk, nprim * d.hstridek * sizeof(double));
+        cudaError_t e = pool_alloc(ctx, nprim * d.hstrideb * sizeof(double), &pl->d.Hb);
+        if (e == cudaSuccess) e = pool_alloc(ctx, nprim * d.hstridek * sizeof(double), &pl->d.Hk);
         if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.scal, nprim * 8 * sizeof(double));
         if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.pairmax, (size_t)npair * sizeof(double));
         if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.ij, (size_t)npair * 2 * sizeof(int));
         if (e == cudaSuccess) e = cudaMemcpy(pl->d.ij, ij, (size_t)npair * 2 * sizeof(int), cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = launch_pair_kernel(ctx, pl->d, 0);
         if (e == cudaSuccess) e = cudaStreamSynchronize(0);
-        if (e != cudaSuccess) { free_pair_storage(pl); return cuda_fail(ctx, "md4_build_pairs", e); }
+        if (e != cudaSuccess) { free_pair_storage(pl, false); return cuda_fail(ctx, "md4_build_pairs", e); }
     }
     ctx->lists.insert(pl);
     *out = pl;
@@ -210,7 +257,9 @@ void md4_free_pairs(md4_ctx* ctx, md4_pairs* pairs) {
     if (it == ctx->lists.end()) return;
     ctx->lists.erase(it);
     DeviceGuard g(ctx->device);
-    free_pair_storage(pairs);
+    // same guarantee cudaFree gave: work that still reads the list has finished before its buffers are reused
+    cudaDeviceSynchronize();
+    free_pair_storage(pairs, true);
 }
 
 int md4_pairs_count(const md4_pairs* pairs) { return pairs ? pairs->d.npair : -1; }

@@ -6,6 +6,7 @@
 #include <string>
 #include <vector>
 #include <set>
+#include <map>
 
 #include "../../include/md4.h"
 
@@ -114,6 +115,10 @@ struct md4_ctx {
     double* d_coef = nullptr;
     std::vector<int> h_l, h_off;
     std::set<md4_pairs*> lists;
+    // freed H buffers kept for the next md4_build_pairs (workspaces grow only, S:8(b)): a batch loop that
+    // builds and frees pair lists every step then never reaches cudaMalloc/cudaFree (both synchronise the device)
+    std::multimap<size_t, void*> pool;
+    size_t pool_bytes = 0;
     double* d_scratch = nullptr;  // md4_compute_host staging
     size_t scratch_doubles = 0;
     long long launches = 0;
