@@ -30,15 +30,8 @@ __device__ __forceinline__ double boys_one(const double* __restrict__ tab, int m
     return r;
 }
 
-// Builds R^{(0)}_{tuv}, t+u+v <= L, for one primitive quartet into Ra[r_addr(t,u,v)] (md4_internal.h).
-// All threads of the CTA must call it.  Rc0/Rc1: two scratch arrays of n_hermite(L) doubles, sS: 32 doubles.
-// srt / sad: shared-memory copies of the Eq.13 table and of the additive address of every graded ordinal
-// (r_tables_to_smem below) -- the table is m-independent, so it is read from shared memory at
-// every level instead of from global memory.
-// scale multiplies every value (K_ab K_cd relative to the pair maxima; 1 in the debug kernel).
-// Level l = 1..L computes [r]^(L-l) for all |r| <= l from level l-1 (one barrier per level, ping-pong
-// buffers instead of the paper's in-place array with two barriers; the last level scatters into the
-// additive layout so that address(p~ + q~) = address(p~) + address(q~), Eq.8 as a pure gather).
+// Shared-memory copies of the Eq.13 table and of the additive address of every graded ordinal: the table is
+// m-independent, so it is read from shared memory at every level instead of from global memory.
 __device__ __forceinline__ void r_tables_to_smem(uint32_t* srt, uint16_t* sad, const uint32_t* __restrict__ rtab,
                                                  const uint32_t* __restrict__ tuv, int L, int tid, int nthr) {
     for (int e = tid; e < n_hermite(L); e += nthr) {
@@ -48,66 +41,73 @@ __device__ __forceinline__ void r_tables_to_smem(uint32_t* srt, uint16_t* sad, c
     }
 }
 
-__device__ __forceinline__ void hermite_r_block(double* Ra, double* Rc0, double* Rc1, double* sS,
-                                                const uint32_t* srt, const uint16_t* sad,
-                                                const double* __restrict__ boys, int L, double zp,
-                                                double Px, double Py, double Pz, double zq, double Qx, double Qy,
-                                                double Qz, double scale, int tid, int nthr) {
+// ---- Hermite Coulomb tensor, built by ONE warp in graded order ------------------------------------
+// hermite_r_warp computes R^{(0)}_{tuv}, t+u+v <= L, of one primitive quartet into GA[graded ordinal]
+// (GA: n_hermite(L) doubles, GB: n_hermite(L-1) doubles of scratch, sS: 32 doubles; all shared memory).
+// Level l = 1..L computes [r]^(L-l) for all |r| <= l from level l-1 (Eq.13; ping-pong buffers and
+// __syncwarp instead of the paper's in-place array with two block barriers); level l lives in
+// GA when L-l is even, so the last level lands in GA.  In the fused kernel the producer warp runs this
+// for the NEXT primitive quartet while the consumer warps contract the current one, calling poll()
+// between batches so that the H_cd ring keeps being refilled; r_scatter() then moves GA into the additive
+// layout (md4_internal.h) with all threads.  scale multiplies every value (K_ab K_cd relative to the pair
+// maxima; 1 in the debug kernel).
+template <class Poll>
+__device__ __forceinline__ void hermite_r_warp(double* GA, double* GB, double* sS, const uint32_t* srt,
+                                               const double* __restrict__ boys, int L, double zp, double Px,
+                                               double Py, double Pz, double zq, double Qx, double Qy, double Qz,
+                                               double scale, int lane, Poll poll) {
     const double X0 = Px - Qx, X1 = Py - Qy, X2 = Pz - Qz;
-    if (tid < 32) {
+    {
         const double zs = zp + zq;
         const double rho = zp * zq / zs;
         const double T = rho * (X0 * X0 + X1 * X1 + X2 * X2);
         // 2 pi^{5/2} = 34.98683665524972497
         const double pref = scale * 34.986836655249724970 / (zp * zq * sqrt(zs));
-        if (tid <= L) {
-            const double F = boys_one(boys, tid, T);
+        if (lane <= L) {
+            const double F = boys_one(boys, lane, T);
             double pw = pref;
             const double m2r = -2.0 * rho;
-            for (int k = 0; k < tid; ++k) pw *= m2r;
-            sS[tid] = pw * F;
+            for (int k = 0; k < lane; ++k) pw *= m2r;
+            sS[lane] = pw * F;
         }
     }
-    __syncthreads();
-    if (L == 0) {
-        if (tid == 0) Ra[0] = sS[0];
-        __syncthreads();
-        return;
-    }
-    double* src = Rc0;
-    double* dst = Rc1;
-    if (tid == 0) src[0] = sS[L];
-    __syncthreads();
-    constexpr int B = 4;  // independent elements in flight per thread
+    __syncwarp();
+    double* src = (L & 1) ? GB : GA;   // level 0
+    double* dst = (L & 1) ? GA : GB;   // level 1
+    if (lane == 0) src[0] = sS[L];
+    __syncwarp();
+    constexpr int B = 4;  // independent elements in flight per lane
     for (int l = 1; l <= L; ++l) {
         const int n = n_hermite(l);
-        const bool last = (l == L);
-        for (int e0 = tid; e0 < n; e0 += B * nthr) {
-            double val[B];
+        for (int e0 = lane; e0 < n; e0 += B * 32) {
+            uint32_t w[B];
 #pragma unroll
             for (int k = 0; k < B; ++k) {
-                const int e = e0 + k * nthr;
-                if (e == 0) {
-                    val[k] = sS[L - l];
-                } else if (e < n) {
-                    const uint32_t w = srt[e];
-                    const int i0 = w & 4095, i1 = (w >> 12) & 4095, C = (w >> 24) & 31, ax = (w >> 29) & 3;
-                    const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
-                    val[k] = fma((double)C, src[i0], x * src[i1]);
-                }
+                const int e = e0 + k * 32;
+                w[k] = srt[e < n ? e : n - 1];
             }
+            double s0[B], s1[B];
+#pragma unroll
+            for (int k = 0; k < B; ++k) { s0[k] = src[w[k] & 4095]; s1[k] = src[(w[k] >> 12) & 4095]; }
 #pragma unroll
             for (int k = 0; k < B; ++k) {
-                const int e = e0 + k * nthr;
-                if (e < n) {
-                    if (last) Ra[sad[e]] = val[k];
-                    else dst[e] = val[k];
-                }
+                const int e = e0 + k * 32;
+                const int ax = (w[k] >> 29) & 3;
+                const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
+                double val = fma((double)((w[k] >> 24) & 31), s0[k], x * s1[k]);
+                if (e == 0) val = sS[L - l];
+                if (e < n) dst[e] = val;
             }
+            poll();
         }
-        __syncthreads();
+        __syncwarp();
         double* t = src; src = dst; dst = t;
     }
+}
+
+// GA (graded order) -> Ra (additive layout); all nthr threads, caller synchronises before and after
+__device__ __forceinline__ void r_scatter(double* Ra, const double* GA, const uint16_t* sad, int L, int tid, int nthr) {
+    for (int e = tid; e < n_hermite(L); e += nthr) Ra[sad[e]] = GA[e];
 }
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -174,6 +174,12 @@ __device__ __forceinline__ void mbar_wait32(uint32_t bar, uint32_t parity) {
         "W_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
         " @p bra D_%=;\n bra W_%=;\n"
         "D_%=:\n}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ bool mbar_test32(uint32_t bar, uint32_t parity) {   // non-blocking
+    uint32_t ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
 }
 __device__ __forceinline__ void bulk_g2s32(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),

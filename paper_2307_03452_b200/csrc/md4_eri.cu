@@ -1,8 +1,11 @@
 // md4_eri.cu -- the fused (ab|cd) kernel: S:8(a) steps a2-a9 in one launch.
 //
 // One CTA works on (one shell quartet) x (a group of 8-row blocks of the bra index ab); one consumer warp
-// owns one 8-row block, one extra warp is the producer of the H_cd ring.  Per primitive quartet the CTA
-// builds the Hermite Coulomb tensor R (Eq.10-13) in shared memory; then every consumer warp, independently,
+// owns one 8-row block, one extra warp is the producer of the H_cd ring AND the builder of the Hermite
+// Coulomb tensor R (Eq.10-13): while the consumers contract primitive quartet i it builds R of primitive
+// quartet i+1 in graded order in its own shared-memory buffers (hermite_r_warp); between two primitive
+// quartets all threads scatter that array into the additive layout (two barriers, ~1 % of the time; the
+// recurrence itself is off the critical path).  Per primitive quartet every consumer warp, independently,
 //   GEMM1 (Eq.14/17):  T[8 x 8*NQT] = H_ab[8 rows, :] . G[:, q~ chunk],
 //          A fragments straight from global/L2, software-prefetched two k-blocks ahead (each H_ab row
 //          block is used by exactly one warp),
@@ -43,17 +46,18 @@ struct EriArgs {
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// Shared memory: R in the additive layout | union { ping-pong scratch of the R recurrence, H_cd ring } |
-// seeds | gather offsets of the p~ and q~ columns | sign bits | mbarriers.
+// Shared memory: R in the additive layout | H_cd ring | graded R of the next primitive quartet (GA) and its
+// ping-pong partner (GB) | seeds | gather offsets of the p~ and q~ columns | sign bits | Eq.13 table |
+// additive address per graded ordinal | mbarriers.
 struct SmemLayout {
-    size_t ra, un, ss, ap, aq, sg, rt, ad, bars, total, stage_bytes, scratch_bytes;
+    size_t ra, un, ga, gb, ss, ap, aq, sg, rt, ad, bars, total, stage_bytes;
     __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst) {
         size_t o = 0;
         ra = o; o += align_up((size_t)r_alloc(L) * 8, 128);
         stage_bytes = (size_t)nrb_cd * 64 * 8;
-        scratch_bytes = align_up((size_t)n_hermite(L) * 8, 16) * 2;
-        const size_t ring = stage_bytes * nst;
-        un = o; o += align_up(ring > scratch_bytes ? ring : scratch_bytes, 128);
+        un = o; o += align_up(stage_bytes * nst, 128);
+        ga = o; o += align_up((size_t)n_hermite(L) * 8, 16);
+        gb = o; o += align_up((size_t)(L > 0 ? n_hermite(L - 1) : 1) * 8, 16);
         ss = o; o += 32 * 8;
         ap = o; o += align_up((size_t)(ncb_p + 1) * 8 * 4, 16);   // one block of slack: the k-loop prefetches
         aq = o; o += align_up((size_t)ncb_q * 8 * 4, 16);
@@ -175,8 +179,8 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
-    double* Rc0 = reinterpret_cast<double*>(smem + lay.un);
-    double* Rc1 = reinterpret_cast<double*>(smem + lay.un + lay.scratch_bytes / 2);
+    double* GA = reinterpret_cast<double*>(smem + lay.ga);
+    double* GB = reinterpret_cast<double*>(smem + lay.gb);
     double* sS = reinterpret_cast<double*>(smem + lay.ss);
     int* ap = reinterpret_cast<int*>(smem + lay.ap);   // byte offset of p~ in Ra, per H_ab column
     int* aq = reinterpret_cast<int*>(smem + lay.aq);   // byte offset of q~ in Ra, per H_cd column
@@ -190,7 +194,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     const int L = a.L;
     const int stage_doubles = a.nrb_cd * 64;
 
-    // R array zeroed once: the recurrence always writes the same addresses, everything else (only ever
+    // R array zeroed once: the scatter always writes the same addresses, everything else (only ever
     // read through padding columns, times a zero of H) stays 0
     for (int i = tid; i < r_alloc(L); i += nthr) Ra[i] = 0.0;
     r_tables_to_smem(srt, sad, a.rtab, a.tuv, L, tid, nthr);
@@ -234,84 +238,108 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     cc.nrb_cd = a.nrb_cd;
     const uint32_t ringbase32 = smem_u32(smem + lay.un);
     RingPos rp{0u, 0u};  // same sequence in every warp
+    const bool producer = (warp == a.wpc);
 
-    for (long long item = blockIdx.x; item < a.nitems; item += gridDim.x) {
+    // builds R of primitive quartet (it, q, p) into GA; poll() is called between batches
+    auto build_r = [&](long long it, int q, int p, auto poll) {
+        const long long qt = it / a.ncta_per_q;
+        const int ib = (int)(qt / a.nket), jk = (int)(qt % a.nket);
+        const double* sp = a.sb + ((size_t)ib * a.Kb + p) * 8;
+        const double* sq = a.sk + ((size_t)jk * a.Kk + q) * 8;
+        hermite_r_warp(GA, GB, sS, srt, a.boys, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
+                       __ldg(sq + 1), __ldg(sq + 2), __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), lane, poll);
+    };
+
+    // primitive quartets of this CTA in order: (item, kq, kp), kp fastest
+    long long item = blockIdx.x;
+    int kq = 0, kp = 0;
+    bool have = item < a.nitems;
+    if (have && producer) build_r(item, 0, 0, [] {});
+
+    double2 acc[NT_CD];
+    while (have) {
+        long long nitem = item;
+        int nkq = kq, nkp = kp + 1;
+        if (nkp == a.Kb) { nkp = 0; if (++nkq == a.Kk) { nkq = 0; nitem += gridDim.x; } }
+        const bool nhave = nitem < a.nitems;
+
         const long long quartet = item / a.ncta_per_q;
         const int ms = (int)(item % a.ncta_per_q);
         const int ib = (int)(quartet / a.nket), jk = (int)(quartet % a.nket);
         const int mbk = ms * a.wpc + warp;       // 8-row block of ab owned by this warp
-        const bool producer = (warp == a.wpc);
         const bool active = !producer && (mbk < a.nrb_ab);
-
-        double2 acc[NT_CD];
+        if (kq == 0 && kp == 0) {
 #pragma unroll
-        for (int i = 0; i < NT_CD; ++i) acc[i] = make_double2(0.0, 0.0);
-
-        for (int kq = 0; kq < a.Kk; ++kq) {
-            const double* sq = a.sk + ((size_t)jk * a.Kk + kq) * 8;
-            const double* Hq = a.Hk + ((size_t)jk * a.Kk + kq) * a.hsk;
-            for (int kp = 0; kp < a.Kb; ++kp) {
-                const double* sp = a.sb + ((size_t)ib * a.Kb + kp) * 8;
-                const double* Hp = a.Hb + ((size_t)ib * a.Kb + kp) * a.hsb;
-                PT_DECL
-                __syncthreads();  // every warp is done with the previous R and with the ring (= R scratch)
-                PT_MARK(4)
-                hermite_r_block(Ra, Rc0, Rc1, sS, srt, sad, a.boys, L, __ldg(sp), __ldg(sp + 1),
-                                __ldg(sp + 2), __ldg(sp + 3), __ldg(sq), __ldg(sq + 1), __ldg(sq + 2),
-                                __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), tid, nthr);
-                if (producer) {
-                    // ---- stream H_cd of this ket primitive through the ring, one column block per stage
-                    if (lane == 0) {
-                        fence_proxy_async();  // the scratch writes of the R recurrence precede the bulk copies
-                        for (int jq = 0; jq < a.ncb_q; ++jq) {
-                            mbar_wait32(cc.empty32 + rp.s * 8u, rp.ph ^ 1u);
-                            mbar_expect_tx32(cc.full32 + rp.s * 8u, cc.stage_bytes);
-                            bulk_g2s32(ringbase32 + rp.s * cc.stage_bytes, Hq + (size_t)jq * stage_doubles, cc.stage_bytes,
-                                       cc.full32 + rp.s * 8u);
-                            rp.advance(cc.nst);
-                        }
-                    }
-                    rp.s = __shfl_sync(0xffffffffu, rp.s, 0);
-                    rp.ph = __shfl_sync(0xffffffffu, rp.ph, 0);
-                    continue;
-                }
-                if (!active) {
-                    // a warp without rows still takes part in the ring protocol
-                    for (int jq = 0; jq < a.ncb_q; ++jq) {
-                        mbar_wait32(cc.full32 + rp.s * 8u, rp.ph);
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive32(cc.empty32 + rp.s * 8u);
-                        rp.advance(cc.nst);
-                    }
-                    continue;
-                }
-                cc.Ablk = Hp + (size_t)mbk * 64 + lane * 2;
-                for (int ch = 0; ch < nchunk; ++ch) {
-                    const int j0 = ch * a.ncb_q / nchunk;
-                    const int nq = (ch + 1) * a.ncb_q / nchunk - j0;
-                    if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
-                    else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
-                    else consume_chunk<NQT - 2, NT_CD, EXACT, true>(acc, cc, j0, nq, rp);
-                }
-            }
+            for (int i = 0; i < NT_CD; ++i) acc[i] = make_double2(0.0, 0.0);
         }
-        // ---- epilogue: common factor K_ab K_cd of the pair maxima, applied in two halves so that
-        // results near the bottom of the FP64 range are still correctly rounded
+
         PT_DECL
-        if (active) {
-            const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
-            const int row = mbk * 8 + (lane >> 2);
-            if (row < a.nab) {
-                double* o = a.out + (size_t)quartet * a.nab * a.ncd + (size_t)row * a.ncd;
+        __syncthreads();  // consumers are done with R of the previous primitive quartet, the builder with GA
+        r_scatter(Ra, GA, sad, L, tid, nthr);
+        __syncthreads();
+        PT_MARK(0)
+
+        if (producer) {
+            // ---- stream H_cd of this ket primitive through the ring, one column block per stage, and build
+            // R of the next primitive quartet in between
+            const double* Hq = a.Hk + ((size_t)jk * a.Kk + kq) * a.hsk;
+            int jq = 0;
+            auto issue = [&] {
+                mbar_expect_tx32(cc.full32 + rp.s * 8u, cc.stage_bytes);
+                bulk_g2s32(ringbase32 + rp.s * cc.stage_bytes, Hq + (size_t)jq * stage_doubles, cc.stage_bytes,
+                           cc.full32 + rp.s * 8u);
+                rp.advance(cc.nst);
+                ++jq;
+            };
+            auto poll = [&] {
+                if (lane == 0)
+                    while (jq < a.ncb_q && mbar_test32(cc.empty32 + rp.s * 8u, rp.ph ^ 1u)) issue();
+            };
+            poll();
+            if (nhave) build_r(nitem, nkq, nkp, poll);
+            if (lane == 0)
+                while (jq < a.ncb_q) {
+                    mbar_wait32(cc.empty32 + rp.s * 8u, rp.ph ^ 1u);
+                    issue();
+                }
+            rp.s = __shfl_sync(0xffffffffu, rp.s, 0);
+            rp.ph = __shfl_sync(0xffffffffu, rp.ph, 0);
+        } else if (!active) {
+            // a warp without rows still takes part in the ring protocol
+            for (int jq = 0; jq < a.ncb_q; ++jq) {
+                mbar_wait32(cc.full32 + rp.s * 8u, rp.ph);
+                __syncwarp();
+                if (lane == 0) mbar_arrive32(cc.empty32 + rp.s * 8u);
+                rp.advance(cc.nst);
+            }
+        } else {
+            const double* Hp = a.Hb + ((size_t)ib * a.Kb + kp) * a.hsb;
+            cc.Ablk = Hp + (size_t)mbk * 64 + lane * 2;
+            for (int ch = 0; ch < nchunk; ++ch) {
+                const int j0 = ch * a.ncb_q / nchunk;
+                const int nq = (ch + 1) * a.ncb_q / nchunk - j0;
+                if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
+                else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
+                else consume_chunk<NQT - 2, NT_CD, EXACT, true>(acc, cc, j0, nq, rp);
+            }
+            // ---- epilogue after the last primitive quartet of the item: common factor K_ab K_cd of the pair
+            // maxima, applied in two halves so that results near the bottom of the FP64 range are still
+            // correctly rounded
+            if (nitem != item) {
+                const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
+                const int row = mbk * 8 + (lane >> 2);
+                if (row < a.nab) {
+                    double* o = a.out + (size_t)quartet * a.nab * a.ncd + (size_t)row * a.ncd;
 #pragma unroll
-                for (int nb = 0; nb < NT_CD; ++nb) {
-                    const int col = nb * 8 + 2 * cc.k4;
-                    if (col < a.ncd) o[col] = (acc[nb].x * f) * f;
-                    if (col + 1 < a.ncd) o[col + 1] = (acc[nb].y * f) * f;
+                    for (int nb = 0; nb < NT_CD; ++nb) {
+                        const int col = nb * 8 + 2 * cc.k4;
+                        if (col < a.ncd) o[col] = (acc[nb].x * f) * f;
+                        if (col + 1 < a.ncd) o[col + 1] = (acc[nb].y * f) * f;
+                    }
                 }
             }
         }
-        PT_MARK(5)
+        item = nitem; kq = nkq; kp = nkp; have = nhave;
     }
 }
 
@@ -398,22 +426,23 @@ __global__ void debug_boys_kernel(const double* tab, int mmax, int n, const doub
     out[i] = boys_one(tab, i % (mmax + 1), T[i / (mmax + 1)]);
 }
 
-// out: dense [(L+1)^3] array, out[(t*(L+1)+u)*(L+1)+v] = R_{tuv} for t+u+v <= L, 0 elsewhere
+// out: dense [(L+1)^3] array, out[(t*(L+1)+u)*(L+1)+v] = R_{tuv} for t+u+v <= L, 0 elsewhere; one warp
 __global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const double* boys, int L, const double* pq,
                                double* out) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int S = L + 1;
     double* Ra = reinterpret_cast<double*>(smem);
-    double* Rc0 = Ra + r_alloc(L);
-    double* Rc1 = Rc0 + n_hermite(L);
-    double* sS = Rc1 + n_hermite(L);
+    double* GA = Ra + r_alloc(L);
+    double* GB = GA + n_hermite(L);
+    double* sS = GB + n_hermite(L);
     uint32_t* srt = reinterpret_cast<uint32_t*>(sS + 32);
     uint16_t* sad = reinterpret_cast<uint16_t*>(srt + n_hermite(L));
     for (int i = threadIdx.x; i < r_alloc(L); i += blockDim.x) Ra[i] = 0.0;
     r_tables_to_smem(srt, sad, rtab, tuv, L, threadIdx.x, blockDim.x);
     __syncthreads();
-    hermite_r_block(Ra, Rc0, Rc1, sS, srt, sad, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7],
-                    1.0, threadIdx.x, blockDim.x);
+    hermite_r_warp(GA, GB, sS, srt, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7], 1.0, threadIdx.x, [] {});
+    __syncthreads();
+    r_scatter(Ra, GA, sad, L, threadIdx.x, blockDim.x);
     __syncthreads();
     for (int i = threadIdx.x; i < S * S * S; i += blockDim.x) {
         const int t = i / (S * S), u = (i / S) % S, v = i % S;
@@ -433,7 +462,7 @@ cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_ou
     const size_t sm = ((size_t)r_alloc(L) + 2 * (size_t)n_hermite(L) + 32) * 8 + (size_t)n_hermite(L) * 6 + 16;
     cudaError_t e = cudaFuncSetAttribute(debug_r_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    debug_r_kernel<<<1, 256, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, L, d_pq, d_out);
+    debug_r_kernel<<<1, 32, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, L, d_pq, d_out);
     ctx->launches++;
     return cudaGetLastError();
 }
