@@ -41,18 +41,22 @@ __device__ __forceinline__ void r_tables_to_smem(uint32_t* srt, uint16_t* sad, c
     }
 }
 
-// ---- Hermite Coulomb tensor, built by ONE warp in graded order ------------------------------------
-// hermite_r_warp computes R^{(0)}_{tuv}, t+u+v <= L, of one primitive quartet into GA[graded ordinal]
-// (GA: n_hermite(L) doubles, GB: n_hermite(L-1) doubles of scratch, sS: 32 doubles; all shared memory).
-// Level l = 1..L computes [r]^(L-l) for all |r| <= l from level l-1 (Eq.13; ping-pong buffers and
-// __syncwarp instead of the paper's in-place array with two block barriers); level l lives in
-// GA when L-l is even, so the last level lands in GA.  In the fused kernel the producer warp runs this
-// for the NEXT primitive quartet while the consumer warps contract the current one, calling poll()
-// between batches so that the H_cd ring keeps being refilled; r_scatter() then moves GA into the additive
-// layout (md4_internal.h) with all threads.  scale multiplies every value (K_ab K_cd relative to the pair
-// maxima; 1 in the debug kernel).
+// ---- Hermite Coulomb tensor, built by ONE warp in graded order, in place ---------------------------
+// hermite_r_warp computes R^{(0)}_{tuv}, t+u+v <= L, of one primitive quartet into G[graded ordinal]
+// (G: n_hermite(L) + L doubles, sS: 32 doubles; shared memory).  As in Listing 3.1 one array
+// serves all levels: level l = 1..L holds [r]^(L-l), |r| <= l, at G[(L-l) + ord(r)], i.e. every level is
+// shifted down by one slot, and is computed from level l-1 by Eq.13.  The slot a value is written to held
+// the level l-1 value of the PREVIOUS ordinal, which only elements with an equal or higher ordinal read:
+// batches of 32*B elements are therefore processed from the top down, all loads of a batch before its
+// stores (__syncwarp) -- one warp needs no block barrier (the paper uses two per level).
+// In the fused kernel the producer warp runs this for the NEXT primitive quartet while the consumer warps
+// contract the current one, calling poll() between batches so that the H_cd ring keeps being refilled;
+// r_scatter() then moves G into the additive layout (md4_internal.h) with all threads.  scale multiplies
+// every value (K_ab K_cd relative to the pair maxima; 1 in the debug kernel).
+__host__ __device__ inline int r_graded_alloc(int L) { return n_hermite(L) + L; }
+
 template <class Poll>
-__device__ __forceinline__ void hermite_r_warp(double* GA, double* GB, double* sS, const uint32_t* srt,
+__device__ __forceinline__ void hermite_r_warp(double* G, double* sS, const uint32_t* srt,
                                                const double* __restrict__ boys, int L, double zp, double Px,
                                                double Py, double Pz, double zq, double Qx, double Qy, double Qz,
                                                double scale, int lane, Poll poll) {
@@ -72,40 +76,43 @@ __device__ __forceinline__ void hermite_r_warp(double* GA, double* GB, double* s
         }
     }
     __syncwarp();
-    double* src = (L & 1) ? GB : GA;   // level 0
-    double* dst = (L & 1) ? GA : GB;   // level 1
-    if (lane == 0) src[0] = sS[L];
+    if (lane == 0) G[L] = sS[L];   // level 0: [0]^(L)
     __syncwarp();
     constexpr int B = 4;  // independent elements in flight per lane
     for (int l = 1; l <= L; ++l) {
         const int n = n_hermite(l);
-        for (int e0 = lane; e0 < n; e0 += B * 32) {
+        const double* src = G + (L - l + 1);
+        double* dst = G + (L - l);
+        const int nbatch = (n + 32 * B - 1) / (32 * B);
+        for (int bt = nbatch - 1; bt >= 0; --bt) {
+            const int e0 = bt * 32 * B + lane;
             uint32_t w[B];
 #pragma unroll
             for (int k = 0; k < B; ++k) {
                 const int e = e0 + k * 32;
                 w[k] = srt[e < n ? e : n - 1];
             }
-            double s0[B], s1[B];
+            double val[B];
 #pragma unroll
-            for (int k = 0; k < B; ++k) { s0[k] = src[w[k] & 4095]; s1[k] = src[(w[k] >> 12) & 4095]; }
+            for (int k = 0; k < B; ++k) {
+                const int ax = (w[k] >> 29) & 3;
+                const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
+                val[k] = fma((double)((w[k] >> 24) & 31), src[w[k] & 4095], x * src[(w[k] >> 12) & 4095]);
+            }
+            __syncwarp();   // every load of the batch precedes its stores
 #pragma unroll
             for (int k = 0; k < B; ++k) {
                 const int e = e0 + k * 32;
-                const int ax = (w[k] >> 29) & 3;
-                const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
-                double val = fma((double)((w[k] >> 24) & 31), s0[k], x * s1[k]);
-                if (e == 0) val = sS[L - l];
-                if (e < n) dst[e] = val;
+                if (e == 0) val[k] = sS[L - l];
+                if (e < n) dst[e] = val[k];
             }
             poll();
         }
         __syncwarp();
-        double* t = src; src = dst; dst = t;
     }
 }
 
-// GA (graded order) -> Ra (additive layout); all nthr threads, caller synchronises before and after
+// G (graded order) -> Ra (additive layout); all nthr threads, caller synchronises before and after
 __device__ __forceinline__ void r_scatter(double* Ra, const double* GA, const uint16_t* sad, int L, int tid, int nthr) {
     for (int e = tid; e < n_hermite(L); e += nthr) Ra[sad[e]] = GA[e];
 }

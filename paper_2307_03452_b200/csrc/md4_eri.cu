@@ -46,18 +46,16 @@ struct EriArgs {
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// Shared memory: R in the additive layout | H_cd ring | graded R of the next primitive quartet (GA) and its
-// ping-pong partner (GB) | seeds | gather offsets of the p~ and q~ columns | sign bits | Eq.13 table |
+// Shared memory: R in the additive layout | H_cd ring | graded R of the next primitive quartet (GA) | seeds | gather offsets of the p~ and q~ columns | sign bits | Eq.13 table |
 // additive address per graded ordinal | mbarriers.
 struct SmemLayout {
-    size_t ra, un, ga, gb, ss, ap, aq, sg, rt, ad, bars, total, stage_bytes;
+    size_t ra, un, ga, ss, ap, aq, sg, rt, ad, bars, total, stage_bytes;
     __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst) {
         size_t o = 0;
         ra = o; o += align_up((size_t)r_alloc(L) * 8, 128);
         stage_bytes = (size_t)nrb_cd * 64 * 8;
         un = o; o += align_up(stage_bytes * nst, 128);
-        ga = o; o += align_up((size_t)n_hermite(L) * 8, 16);
-        gb = o; o += align_up((size_t)(L > 0 ? n_hermite(L - 1) : 1) * 8, 16);
+        ga = o; o += align_up((size_t)r_graded_alloc(L) * 8, 16);
         ss = o; o += 32 * 8;
         ap = o; o += align_up((size_t)(ncb_p + 1) * 8 * 4, 16);   // one block of slack: the k-loop prefetches
         aq = o; o += align_up((size_t)ncb_q * 8 * 4, 16);
@@ -180,7 +178,6 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
     double* GA = reinterpret_cast<double*>(smem + lay.ga);
-    double* GB = reinterpret_cast<double*>(smem + lay.gb);
     double* sS = reinterpret_cast<double*>(smem + lay.ss);
     int* ap = reinterpret_cast<int*>(smem + lay.ap);   // byte offset of p~ in Ra, per H_ab column
     int* aq = reinterpret_cast<int*>(smem + lay.aq);   // byte offset of q~ in Ra, per H_cd column
@@ -246,7 +243,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
         const int ib = (int)(qt / a.nket), jk = (int)(qt % a.nket);
         const double* sp = a.sb + ((size_t)ib * a.Kb + p) * 8;
         const double* sq = a.sk + ((size_t)jk * a.Kk + q) * 8;
-        hermite_r_warp(GA, GB, sS, srt, a.boys, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
+        hermite_r_warp(GA, sS, srt, a.boys, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
                        __ldg(sq + 1), __ldg(sq + 2), __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), lane, poll);
     };
 
@@ -433,14 +430,13 @@ __global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const 
     const int S = L + 1;
     double* Ra = reinterpret_cast<double*>(smem);
     double* GA = Ra + r_alloc(L);
-    double* GB = GA + n_hermite(L);
-    double* sS = GB + n_hermite(L);
+    double* sS = GA + 2 * n_hermite(L);
     uint32_t* srt = reinterpret_cast<uint32_t*>(sS + 32);
     uint16_t* sad = reinterpret_cast<uint16_t*>(srt + n_hermite(L));
     for (int i = threadIdx.x; i < r_alloc(L); i += blockDim.x) Ra[i] = 0.0;
     r_tables_to_smem(srt, sad, rtab, tuv, L, threadIdx.x, blockDim.x);
     __syncthreads();
-    hermite_r_warp(GA, GB, sS, srt, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7], 1.0, threadIdx.x, [] {});
+    hermite_r_warp(GA, sS, srt, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7], 1.0, threadIdx.x, [] {});
     __syncthreads();
     r_scatter(Ra, GA, sad, L, threadIdx.x, blockDim.x);
     __syncthreads();
