@@ -139,6 +139,12 @@ md4_status md4_create(md4_ctx** out, int cuda_device) {
             c->tab.solid_lo[l] = d;
         }
     }
+    if (e == cudaSuccess) {
+        // partial [ab|q~] of contracted bras: one slab per CTA of the persistent fused kernel (L2 resident)
+        void* t = nullptr;
+        e = cudaMalloc(&t, (size_t)c->num_sms * TACC_WARPS * TACC_QBLOCKS * 64 * sizeof(double));
+        if (e == cudaSuccess) { c->table_allocs.push_back(t); c->d_tacc = static_cast<double*>(t); }
+    }
     if (e != cudaSuccess) {
         g_create_err = std::string("md4_create: table upload: ") + cudaGetErrorString(e);
         for (void* p : c->table_allocs) cudaFree(p);

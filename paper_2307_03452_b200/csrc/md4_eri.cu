@@ -40,6 +40,7 @@ struct EriArgs {
     int L, wpc, ncta_per_q, nst;
     long long nitems;
     const uint32_t* rtab; const uint32_t* tuv; const double* boys;
+    double* tacc;   // [grid][wpc][ncb_q][32][2] partial [ab|q~] of contracted bras
     const uint32_t* colp; const uint32_t* colq;   // bra-order columns of the bra class, ket-order columns of the ket class
     double* out;
 };
@@ -99,19 +100,24 @@ struct ConsumerCtx {
     uint32_t full32, empty32;
     uint32_t stage_bytes, nst;
     int ncb_p, nrb_cd, k4, lane;
+    double* tacc;          // this lane's slot of the [ab|q~] scratch of its warp (q-block 0), contracted bras only
 };
 
 // One chunk of NQ q~ blocks for one warp: T = H_ab[8 rows] . G[:, chunk] (GEMM1), then
 // acc += (sign . T) . H_cd[:, chunk]^T (GEMM2) against the ring.  PRED: q-blocks n >= nq are skipped
 // (general classes); otherwise nq == NQ.  EXACT: nrb_cd == NT_CD.
 template <int NQ, int NT_CD, bool EXACT, bool PRED>
-__device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const ConsumerCtx& c, int j0, int nq, RingPos& rp) {
+__device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const ConsumerCtx& c, int j0, int nq, RingPos& rp,
+                                              bool load_t, bool last_kp) {
     double2 T[NQ];
     uint32_t aqr[NQ];
     PT_DECL
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
-        T[n] = make_double2(0.0, 0.0);
+        // [ab|q~] accumulates over the bra primitives (Listing 2.1 line 7): from the second one on the
+        // accumulators start from the sum so far, kept in an L2-resident scratch in fragment layout
+        T[n] = (load_t && (!PRED || n < nq)) ? *reinterpret_cast<const double2*>(c.tacc + (size_t)(j0 + n) * 64)
+                                             : make_double2(0.0, 0.0);
         aqr[n] = c.ra32 + ((!PRED || n < nq) ? lds_u32(c.aq32 + (uint32_t)(j0 + n) * 32u) : 0u);
     }
     // ---- GEMM1: the B operand is G[p~,q~] = +-R[p~+q~] read at address(p~) + address(q~) (Eq.8)
@@ -139,6 +145,13 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
             if (!PRED || n < nq) dmma884(T[n].x, T[n].y, av.y, b[n]);
     }
     PT_MARK(1)
+    if (!last_kp) {
+        // more bra primitives to come: park the partial [ab|q~]; the ket transform runs once per ket primitive
+#pragma unroll
+        for (int n = 0; n < NQ; ++n)
+            if (!PRED || n < nq) *reinterpret_cast<double2*>(c.tacc + (size_t)(j0 + n) * 64) = T[n];
+        return;
+    }
     // ---- sign of Eq.8 and GEMM2: acc += T . H_cd[:, chunk]^T
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
@@ -233,6 +246,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
     cc.nst = (uint32_t)a.nst;
     cc.ncb_p = a.ncb_p;
     cc.nrb_cd = a.nrb_cd;
+    cc.tacc = a.tacc + (((size_t)blockIdx.x * a.wpc + (warp < a.wpc ? warp : 0)) * a.ncb_q * 32 + lane) * 2;
     const uint32_t ringbase32 = smem_u32(smem + lay.un);
     RingPos rp{0u, 0u};  // same sequence in every warp
     const bool producer = (warp == a.wpc);
@@ -276,11 +290,12 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
         __syncthreads();
         PT_MARK(0)
 
+        const bool last_kp = (kp == a.Kb - 1);   // the ket transform (and the ring) run with the last bra primitive only
         if (producer) {
             // ---- stream H_cd of this ket primitive through the ring, one column block per stage, and build
             // R of the next primitive quartet in between
             const double* Hq = a.Hk + ((size_t)jk * a.Kk + kq) * a.hsk;
-            int jq = 0;
+            int jq = last_kp ? 0 : a.ncb_q;
             auto issue = [&] {
                 mbar_expect_tx32(cc.full32 + rp.s * 8u, cc.stage_bytes);
                 bulk_g2s32(ringbase32 + rp.s * cc.stage_bytes, Hq + (size_t)jq * stage_doubles, cc.stage_bytes,
@@ -303,7 +318,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
             rp.ph = __shfl_sync(0xffffffffu, rp.ph, 0);
         } else if (!active) {
             // a warp without rows still takes part in the ring protocol
-            for (int jq = 0; jq < a.ncb_q; ++jq) {
+            for (int jq = last_kp ? 0 : a.ncb_q; jq < a.ncb_q; ++jq) {
                 mbar_wait32(cc.full32 + rp.s * 8u, rp.ph);
                 __syncwarp();
                 if (lane == 0) mbar_arrive32(cc.empty32 + rp.s * 8u);
@@ -315,9 +330,9 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
             for (int ch = 0; ch < nchunk; ++ch) {
                 const int j0 = ch * a.ncb_q / nchunk;
                 const int nq = (ch + 1) * a.ncb_q / nchunk - j0;
-                if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
-                else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false>(acc, cc, j0, nq, rp);
-                else consume_chunk<NQT - 2, NT_CD, EXACT, true>(acc, cc, j0, nq, rp);
+                if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false>(acc, cc, j0, nq, rp, kp > 0, last_kp);
+                else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false>(acc, cc, j0, nq, rp, kp > 0, last_kp);
+                else consume_chunk<NQT - 2, NT_CD, EXACT, true>(acc, cc, j0, nq, rp, kp > 0, last_kp);
             }
             // ---- epilogue after the last primitive quartet of the item: common factor K_ab K_cd of the pair
             // maxima, applied in two halves so that results near the bottom of the FP64 range are still
@@ -390,6 +405,7 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     a.rtab = ctx->tab.rtab; a.tuv = ctx->tab.tuv; a.boys = ctx->tab.boys;
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];
     a.out = d_out;
+    a.tacc = ctx->d_tacc;
     const int nt = a.nrb_cd;
     // exact instantiations for the ket classes of l >= 4 shells (N_cd = 81, 99, 117, 121, 143, 169); the
     // others (no product of two odd numbers <= 13 falls in 14, 17, 19-21 row blocks) run predicated

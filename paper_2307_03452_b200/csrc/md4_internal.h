@@ -47,6 +47,8 @@ constexpr int RS2 = 631;
 __host__ __device__ inline int r_addr(int t, int u, int v) { return t * RS2 + u * RS1 + v; }
 __host__ __device__ inline int r_alloc(int L) { return L * RS2 + 32; }  // doubles; +32: padding columns read addresses 0..15 past the largest p~
 constexpr int LPAIR = 2 * LMAX;          // highest l_a + l_b of a shell pair
+constexpr int TACC_WARPS = 11;            // consumer warps per CTA of the fused kernel, at most
+constexpr int TACC_QBLOCKS = 64;         // q~ column blocks, at most (57 for l_pair = 12)
 constexpr uint32_t COL_PAD = 1u << 31;   // flag of a padding column in the column tables
 
 // Constant device tables, built once per context (md4_tables.cpp).
@@ -119,6 +121,7 @@ struct md4_ctx {
     // builds and frees pair lists every step then never reaches cudaMalloc/cudaFree (both synchronise the device)
     std::multimap<size_t, void*> pool;
     size_t pool_bytes = 0;
+    double* d_tacc = nullptr;     // partial [ab|q~] of contracted bras, one slab per CTA of the fused kernel (md4_eri.cu)
     double* d_scratch = nullptr;  // md4_compute_host staging
     size_t scratch_doubles = 0;
     long long launches = 0;
