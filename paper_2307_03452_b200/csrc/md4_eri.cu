@@ -38,7 +38,9 @@ struct EriArgs {
     int Kb, Kk, nbra, nket;
     int nab, ncd, nrb_ab, nrb_cd, ncb_p, ncb_q;
     int L, wpc, ncta_per_q, nst;
-    long long nitems;
+    int row0[3], nrows[3];   // 8-row blocks of ab of the ncta_per_q work items of one quartet (plan_items)
+    long long nquartets;
+    int qmajor;   // 1: a CTA takes whole quartets (items of unequal size); 0: the items of a quartet go to neighbouring CTAs
     const uint32_t* rtab; const uint32_t* tuv; const double* boys;
     double* tacc;   // [grid][wpc][ncb_q][32][2] partial [ab|q~] of contracted bras
     const uint32_t* colp; const uint32_t* colq;   // bra-order columns of the bra class, ket-order columns of the ket class
@@ -253,7 +255,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
 
     // builds R of primitive quartet (it, q, p) into GA; poll() is called between batches
     auto build_r = [&](long long it, int q, int p, auto poll) {
-        const long long qt = it / a.ncta_per_q;
+        const long long qt = it;
         const int ib = (int)(qt / a.nket), jk = (int)(qt % a.nket);
         const double* sp = a.sb + ((size_t)ib * a.Kb + p) * 8;
         const double* sq = a.sk + ((size_t)jk * a.Kk + q) * 8;
@@ -261,24 +263,38 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                        __ldg(sq + 1), __ldg(sq + 2), __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), lane, poll);
     };
 
-    // primitive quartets of this CTA in order: (item, kq, kp), kp fastest
-    long long item = blockIdx.x;
+    // primitive quartets of this CTA in order: (quartet, item of the quartet, kq, kp), kp fastest.  A CTA takes
+    // whole quartets, so that every CTA gets the same mix of item sizes
+    // (equal items: neighbouring CTAs share a quartet, which halves the number of H_cd matrices in flight in L2)
+    long long quartet = a.qmajor ? (long long)blockIdx.x : (long long)(blockIdx.x / a.ncta_per_q);
+    int ms = a.qmajor ? 0 : (int)(blockIdx.x % a.ncta_per_q);
     int kq = 0, kp = 0;
-    bool have = item < a.nitems;
-    if (have && producer) build_r(item, 0, 0, [] {});
+    bool have = quartet < a.nquartets;
+    if (have && producer) build_r(quartet, 0, 0, [] {});
 
     double2 acc[NT_CD];
     while (have) {
-        long long nitem = item;
-        int nkq = kq, nkp = kp + 1;
-        if (nkp == a.Kb) { nkp = 0; if (++nkq == a.Kk) { nkq = 0; nitem += gridDim.x; } }
-        const bool nhave = nitem < a.nitems;
+        long long nquartet = quartet;
+        int nms = ms, nkq = kq, nkp = kp + 1;
+        if (nkp == a.Kb) {
+            nkp = 0;
+            if (++nkq == a.Kk) {
+                nkq = 0;
+                if (a.qmajor) {
+                    if (++nms == a.ncta_per_q) { nms = 0; nquartet += gridDim.x; }
+                } else {
+                    const long long g = quartet * a.ncta_per_q + ms + gridDim.x;
+                    nquartet = g / a.ncta_per_q;
+                    nms = (int)(g % a.ncta_per_q);
+                }
+            }
+        }
+        const bool nhave = nquartet < a.nquartets;
+        const bool item_ends = (nquartet != quartet) || (nms != ms);
 
-        const long long quartet = item / a.ncta_per_q;
-        const int ms = (int)(item % a.ncta_per_q);
         const int ib = (int)(quartet / a.nket), jk = (int)(quartet % a.nket);
-        const int mbk = ms * a.wpc + warp;       // 8-row block of ab owned by this warp
-        const bool active = !producer && (mbk < a.nrb_ab);
+        const int mbk = (ms == 0 ? a.row0[0] : (ms == 1 ? a.row0[1] : a.row0[2])) + warp;   // 8-row block of ab owned by this warp
+        const bool active = !producer && warp < (ms == 0 ? a.nrows[0] : (ms == 1 ? a.nrows[1] : a.nrows[2]));
         if (kq == 0 && kp == 0) {
 #pragma unroll
             for (int i = 0; i < NT_CD; ++i) acc[i] = make_double2(0.0, 0.0);
@@ -308,7 +324,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                     while (jq < a.ncb_q && mbar_test32(cc.empty32 + rp.s * 8u, rp.ph ^ 1u)) issue();
             };
             poll();
-            if (nhave) build_r(nitem, nkq, nkp, poll);
+            if (nhave) build_r(nquartet, nkq, nkp, poll);
             if (lane == 0)
                 while (jq < a.ncb_q) {
                     mbar_wait32(cc.empty32 + rp.s * 8u, rp.ph ^ 1u);
@@ -337,7 +353,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
             // ---- epilogue after the last primitive quartet of the item: common factor K_ab K_cd of the pair
             // maxima, applied in two halves so that results near the bottom of the FP64 range are still
             // correctly rounded
-            if (nitem != item) {
+            if (item_ends) {
                 const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
                 const int row = mbk * 8 + (lane >> 2);
                 if (row < a.nab) {
@@ -351,8 +367,27 @@ __global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
                 }
             }
         }
-        item = nitem; kq = nkq; kp = nkp; have = nhave;
+        quartet = nquartet; ms = nms; kq = nkq; kp = nkp; have = nhave;
     }
+}
+
+// Splits the nrb_ab eight-row blocks of a quartet into work items of at most 11 blocks (one consumer warp
+// each).  The FP64 tensor pipe is per SM sub-partition (profiles/r1_fp64_peak.txt) and warp w runs on
+// sub-partition w % 4, so an item of n blocks takes ceil(n/4) block-times: the split minimises their sum
+// (18 blocks: 10 + 8 -> 3 + 2, not 9 + 9 -> 3 + 3), then the number of consumer warps.
+void plan_items(EriArgs& a) {
+    const int n = a.nrb_ab;
+    for (int t = 0; t < 3; ++t) { a.row0[t] = 0; a.nrows[t] = 0; }
+    if (n <= 11) { a.ncta_per_q = 1; a.nrows[0] = n; a.wpc = n; return; }
+    int best = 1 << 30, b1 = 0;
+    for (int n1 = (n + 1) / 2; n1 <= 11; ++n1) {
+        const int n2 = n - n1;
+        const int cost = ((n1 + 3) / 4 + (n2 + 3) / 4) * 16 + n1;
+        if (cost < best) { best = cost; b1 = n1; }
+    }
+    a.ncta_per_q = 2;
+    a.nrows[0] = b1; a.row0[1] = b1; a.nrows[1] = n - b1;
+    a.wpc = b1;
 }
 
 template <int NT_CD, int NQT, int MAXW, bool EXACT>
@@ -371,7 +406,8 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
     auto kern = eri_kernel<NT_CD, NQT, MAXW, EXACT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lay.total);
     if (e != cudaSuccess) { ctx->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return MD4_ECUDA; }
-    long long grid = a.nitems < (long long)ctx->num_sms ? a.nitems : (long long)ctx->num_sms;
+    const long long nwork = a.qmajor ? a.nquartets : a.nquartets * a.ncta_per_q;
+    long long grid = nwork < (long long)ctx->num_sms ? nwork : (long long)ctx->num_sms;
     kern<<<(unsigned)grid, (a.wpc + 1) * 32, lay.total, st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();
@@ -396,11 +432,9 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     a.nab = bra.nab; a.ncd = ket.nab; a.nrb_ab = bra.nrb; a.nrb_cd = ket.nrb;
     a.ncb_p = bra.ncbb; a.ncb_q = ket.ncbk;
     a.L = bra.lsum + ket.lsum;
-    // consumer warps per CTA = 8-row blocks per CTA (<= 11, plus the producer warp); a quartet is split
-    // over ncta_per_q CTAs
-    a.ncta_per_q = (a.nrb_ab + 10) / 11;
-    a.wpc = (a.nrb_ab + a.ncta_per_q - 1) / a.ncta_per_q;
-    a.nitems = (long long)a.nbra * a.nket * a.ncta_per_q;
+    plan_items(a);
+    a.nquartets = (long long)a.nbra * a.nket;
+    a.qmajor = (a.ncta_per_q == 2 && a.nrows[0] != a.nrows[1]) ? 1 : 0;
     a.nst = 2;
     a.rtab = ctx->tab.rtab; a.tuv = ctx->tab.tuv; a.boys = ctx->tab.boys;
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];
