@@ -104,7 +104,9 @@ md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket,
 
 /* Same through HOST buffers (the end-to-end path bench.py's "e2e" times): copies the result to
  * h_out [capacity_doubles] (HOST) through an internal device buffer that grows on demand, and
- * synchronises the stream before returning. */
+ * synchronises before returning.  Large batches are computed in slices of the bra list; the copy of a slice
+ * (internal copy stream) overlaps the kernel of the next one, so with a pinned h_out the call takes
+ * max(compute, PCIe transfer) rather than their sum.  Pageable h_out works, without the overlap. */
 md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* h_out,
                             size_t capacity_doubles, void* cuda_stream);
 

@@ -164,6 +164,10 @@ void md4_destroy(md4_ctx* ctx) {
     pool_release(ctx);
     free_shells(ctx);
     cudaFree(ctx->d_scratch);
+    if (ctx->copy_stream) {
+        for (int i = 0; i < md4_ctx::NSLICE_EV; ++i) cudaEventDestroy(ctx->slice_ev[i]);
+        cudaStreamDestroy(ctx->copy_stream);
+    }
     for (void* p : ctx->table_allocs) cudaFree(p);
     delete ctx;
 }
@@ -328,10 +332,41 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
         if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
         ctx->scratch_doubles = need;
     }
-    s = launch_eri(ctx, bra->d, ket->d, ctx->d_scratch, st);
-    if (s != MD4_OK) return s;
-    cudaError_t e = cudaMemcpyAsync(h_out, ctx->d_scratch, need * sizeof(double), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    // The bra list is cut into slices: the copy of slice i to the host (copy stream) runs under the kernel of
+    // slice i+1 (caller's stream).  out is bra-major, so a slice is one contiguous range of it.  With a pinned
+    // h_out the call is bound by max(compute, PCIe) instead of their sum.
+    if (!ctx->copy_stream) {
+        cudaError_t e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+        for (int i = 0; i < md4_ctx::NSLICE_EV && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&ctx->slice_ev[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
+    }
+    const size_t per_bra = need / (size_t)bra->d.npair;
+    int nslice = 1;
+    if (need * sizeof(double) >= ((size_t)64 << 20)) nslice = bra->d.npair < md4_ctx::NSLICE_EV ? bra->d.npair : md4_ctx::NSLICE_EV;
+    const int kk = bra->d.Ki * bra->d.Kj;
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < nslice && e == cudaSuccess; ++i) {
+        const int b0 = (int)((long long)bra->d.npair * i / nslice), b1 = (int)((long long)bra->d.npair * (i + 1) / nslice);
+        if (b1 == b0) continue;
+        PairListDev sub = bra->d;
+        sub.npair = b1 - b0;
+        sub.Hb += (size_t)b0 * kk * sub.hstrideb;
+        sub.Hk += (size_t)b0 * kk * sub.hstridek;
+        sub.scal += (size_t)b0 * kk * 8;
+        sub.pairmax += b0;
+        sub.ij += 2 * (size_t)b0;
+        double* d_slice = ctx->d_scratch + (size_t)b0 * per_bra;
+        s = launch_eri(ctx, sub, ket->d, d_slice, st);
+        if (s != MD4_OK) { cudaStreamSynchronize(st); cudaStreamSynchronize(ctx->copy_stream); return s; }
+        e = cudaEventRecord(ctx->slice_ev[i], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->slice_ev[i], 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(h_out + (size_t)b0 * per_bra, d_slice, (size_t)(b1 - b0) * per_bra * sizeof(double),
+                                cudaMemcpyDeviceToHost, ctx->copy_stream);
+    }
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaError_t e3 = cudaStreamSynchronize(ctx->copy_stream);
+    if (e == cudaSuccess) e = e2 != cudaSuccess ? e2 : e3;
     if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
     return MD4_OK;
 }

@@ -124,6 +124,9 @@ struct md4_ctx {
     double* d_tacc = nullptr;     // partial [ab|q~] of contracted bras, one slab per CTA of the fused kernel (md4_eri.cu)
     double* d_scratch = nullptr;  // md4_compute_host staging
     size_t scratch_doubles = 0;
+    static constexpr int NSLICE_EV = 8;   // md4_compute_host: bra slices whose D2H copy overlaps the next slice's kernel
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t slice_ev[NSLICE_EV] = {};
     long long launches = 0;
     int num_sms = 0;
     int smem_optin = 0;
