@@ -15,7 +15,7 @@ constexpr int ESZ = NA1 * NA1 * NT1;   // 637 per axis
 constexpr int NCMAX = (LMAX + 1) * (LMAX + 2) / 2;  // 28
 constexpr int NSMAX = 2 * LMAX + 1;    // 13
 constexpr int PAIR_THREADS = 256;
-constexpr int PAIR_SPLIT = 4;          // CTAs per primitive pair (each takes a range of Hermite column blocks)
+constexpr int PAIR_SPLIT = 8;          // CTAs per primitive pair (each takes a range of Hermite column blocks)
 
 // ---- double-double arithmetic (error-free transformations; __d*_rn blocks FMA contraction) ---------
 // Why: H = C_la (x) C_lb E cancels the radial contaminants of the Cartesian Gaussians.  For a tight
