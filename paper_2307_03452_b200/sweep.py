@@ -1,6 +1,6 @@
 """Per-class throughput report over the BASELINE.json configs (config 5's "per-class quartets/s and % of FP64 peak").
 
-    python -m paper_2307_03452_b200.sweep [--configs cfg1,cfg2,cfg3,cfg4,cfg5] [--reps 5] [--out report.md]
+    python -m paper_2307_03452_b200.sweep [--configs cfg1,cfg2,cfg3,cfg4,cfg5,low] [--reps 5] [--out report.md]
 
 For every workload: pair lists are built once (timed separately, the paper excludes H from the quartet loop,
 PAPER.md:146, :158), then md4_compute is timed alone with CUDA events on its stream (3 warm-ups, `reps` repetitions,
@@ -30,6 +30,10 @@ def workloads(names):
             yield inputs.config3()
         elif n == "cfg4":
             yield inputs.config4()
+        elif n == "low":
+            # the remaining classes of the paper's Table 1, same recipe as cfg2
+            yield inputs._perm_config("low (dd|dd) K=1", 11, 64, 2, 10.0, 0.05, 50.0, 64)
+            yield inputs._perm_config("low (ff|ff) K=1", 12, 64, 3, 10.0, 0.05, 50.0, 64)
         elif n == "cfg5":
             for K in (1, 3):
                 for ci in range(len(inputs.sweep_classes())):

@@ -311,3 +311,21 @@ def test_compute_host_matches_device(eng):
     n0 = eng.launch_count()
     eng.compute(bra, ket, out=d)
     assert eng.launch_count() == n0 + 1
+
+
+def test_compute_host_sliced_matches_device(eng):
+    """A batch large enough (cfg2, 480 MB) for md4_compute_host to cut the bra list into slices whose D2H copy
+    overlaps the next slice's kernel: bit-identical to the one-launch device result, ragged last slice included."""
+    import torch
+
+    wl = inputs.config2()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    bra, ket = eng.build_pairs(wl.bra_ij[:61]), eng.build_pairs(wl.ket_ij)   # 61 bra pairs: slices of 7 and 8
+    d = eng.compute(bra, ket)
+    torch.cuda.synchronize()
+    n0 = eng.launch_count()
+    h = eng.compute_host(bra, ket)
+    assert eng.launch_count() - n0 == 8
+    assert np.array_equal(d.cpu().numpy(), h)
+    bra.free(); ket.free()
