@@ -200,11 +200,19 @@ def run_gpu(args):
     import torch
     import torch.distributed as dist
 
+    from paper_2307_03452_b200 import build as md4_build
     from paper_2307_03452_b200 import md4
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if local == 0:
+        md4_build.ensure_built()   # a checkout has no build artefacts; the kernels themselves have no fallback
+    else:
+        for _ in range(600):       # the other local ranks wait for rank 0's build
+            if os.path.exists(md4_build.LIB):
+                break
+            time.sleep(0.5)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the MD4 path has no CPU fallback")
     torch.cuda.set_device(local)

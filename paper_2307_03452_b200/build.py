@@ -62,5 +62,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def ensure_built() -> str:
+    """Compile libmd4.so if it is not there (a checkout without build artefacts); never a fallback for the kernels."""
+    return LIB if os.path.exists(LIB) else build(force=True)
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
