@@ -160,11 +160,15 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
     const double wgt = a.coef[a.off[si] + ka] * a.coef[a.off[sj] + kb];
     const int jb0 = (int)((long long)split * a.ncb / PAIR_SPLIT), jb1 = (int)((long long)(split + 1) * a.ncb / PAIR_SPLIT);
     for (int jb = jb0; jb < jb1; ++jb) {
-        // half transform over b: Y[ac][mb][pp] = sum_bc Cb[mb][bc] Ex Ey Ez
-        for (int idx = tid; idx < nca * nsb * 8; idx += nthr) {
-            const int pp = idx & 7, mb = (idx >> 3) % nsb, ac = (idx >> 3) / nsb;
+        // half transform over b: Y[ac][mb][pp] = sum_bc Cb[mb][bc] Ex Ey Ez.  One thread per (ac, pp) keeps the
+        // 2 lb + 1 sums in registers, so each product Ex Ey Ez is formed once; zero coefficients of the (sparse)
+        // solid-harmonic table are skipped (the test is uniform over the warp: mb and bc do not depend on the lane)
+        for (int idx = tid; idx < nca * 8; idx += nthr) {
+            const int pp = idx & 7, ac = idx >> 3;
             const int col = jb * 8 + pp;
-            dd acc = make_double2(0.0, 0.0);
+            dd acc[NSMAX];
+#pragma unroll
+            for (int mb = 0; mb < NSMAX; ++mb) acc[mb] = make_double2(0.0, 0.0);
             const uint32_t w = a.colb[col];
             if (!(w & COL_PAD)) {
                 const int t = w & 255, u = (w >> 8) & 255, v = (w >> 16) & 255;
@@ -174,10 +178,18 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
                     if (t > ax + bx || u > ay + by || v > az + bz) continue;
                     const dd e3 = dd_mul(dd_mul(sm.E[0][(ax * NA1 + bx) * NT1 + t], sm.E[1][(ay * NA1 + by) * NT1 + u]),
                                          sm.E[2][(az * NA1 + bz) * NT1 + v]);
-                    acc = dd_add(acc, dd_mul(sm.Cb[mb * ncbt + bc], e3));
+#pragma unroll
+                    for (int mb = 0; mb < NSMAX; ++mb) {
+                        if (mb < nsb) {
+                            const dd cb = sm.Cb[mb * ncbt + bc];
+                            if (cb.x != 0.0) acc[mb] = dd_add(acc[mb], dd_mul(cb, e3));
+                        }
+                    }
                 }
             }
-            sm.Y[idx] = acc;
+#pragma unroll
+            for (int mb = 0; mb < NSMAX; ++mb)
+                if (mb < nsb) sm.Y[(ac * nsb + mb) * 8 + pp] = acc[mb];
         }
         __syncthreads();
         // half transform over a, contraction weight, blocked store
@@ -188,7 +200,10 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
             const int pp = idx & 7, row = idx >> 3;
             const int ma = row / nsb, mb = row % nsb;
             dd acc = make_double2(0.0, 0.0);
-            for (int ac = 0; ac < nca; ++ac) acc = dd_add(acc, dd_mul(sm.Ca[ma * nca + ac], sm.Y[(ac * nsb + mb) * 8 + pp]));
+            for (int ac = 0; ac < nca; ++ac) {
+                const dd ca = sm.Ca[ma * nca + ac];
+                if (ca.x != 0.0) acc = dd_add(acc, dd_mul(ca, sm.Y[(ac * nsb + mb) * 8 + pp]));
+            }
             const double h = wgt * acc.x + wgt * acc.y;
             Hp[(row >> 3) * 64 + (row & 7) * 8 + pp] = h;
             const int ck = a.b2k[jb * 8 + pp];
