@@ -187,8 +187,8 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
     PT_MARK(2)
 }
 
-template <int NT_CD, int NQT, int MAXW, bool EXACT>
-__global__ void __launch_bounds__(MAXW * 32, 1) eri_kernel(const EriArgs a) {
+template <int NT_CD, int NQT, int MAXW, bool EXACT, int MINB>
+__global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
@@ -390,24 +390,30 @@ void plan_items(EriArgs& a) {
     a.wpc = b1;
 }
 
-template <int NT_CD, int NQT, int MAXW, bool EXACT>
+// MINB CTAs per SM: small classes (few row blocks, small R) are latency-bound per work item -- two barriers, TMA
+// and L2 round trips around a few dozen DMMAs -- so two or three CTAs share an SM there.
+template <int NT_CD, int NQT, int MAXW, bool EXACT, int MINB>
 md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
+    // shared memory per CTA: the SM's 228 kB less 1 kB reserved per resident CTA
+    const size_t budget = MINB == 1 ? (size_t)ctx->smem_optin : (size_t)(ctx->smem_optin + 1024) / MINB - 1024;
     // ring depth: whatever shared memory is left after R, at least 2 stages, at most MAX_STAGES
     int nst = 2;
     for (int s = MAX_STAGES; s >= 2; --s)
-        if (SmemLayout(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, s).total <= (size_t)ctx->smem_optin) { nst = s; break; }
+        if (SmemLayout(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, s).total <= budget) { nst = s; break; }
     if (nst > a.ncb_q) nst = a.ncb_q < 2 ? 2 : a.ncb_q;
     a.nst = nst;
     const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, nst);
-    if (lay.total > (size_t)ctx->smem_optin) {
+    if (lay.total > budget) {
+        if (MINB > 1) return launch_one<NT_CD, NQT, MAXW, EXACT, 1>(ctx, a, st);
         ctx->err = "md4_compute: shared memory needed exceeds the device limit";
         return MD4_EUNSUPPORTED;
     }
-    auto kern = eri_kernel<NT_CD, NQT, MAXW, EXACT>;
+    auto kern = eri_kernel<NT_CD, NQT, MAXW, EXACT, MINB>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lay.total);
     if (e != cudaSuccess) { ctx->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return MD4_ECUDA; }
     const long long nwork = a.qmajor ? a.nquartets : a.nquartets * a.ncta_per_q;
-    long long grid = nwork < (long long)ctx->num_sms ? nwork : (long long)ctx->num_sms;
+    const long long slots = (long long)ctx->num_sms * MINB;
+    long long grid = nwork < slots ? nwork : slots;
     kern<<<(unsigned)grid, (a.wpc + 1) * 32, lay.total, st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();
@@ -417,8 +423,16 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
 
 template <int NT_CD, bool EXACT>
 md4_status launch_w(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
-    if (a.wpc + 1 <= 9) return launch_one<NT_CD, 8, 9, EXACT>(ctx, a, st);
-    return launch_one<NT_CD, 8, 12, EXACT>(ctx, a, st);
+    if (a.wpc + 1 <= 9) return launch_one<NT_CD, 8, 9, EXACT, 1>(ctx, a, st);
+    return launch_one<NT_CD, 8, 12, EXACT, 1>(ctx, a, st);
+}
+
+// small classes: at most 7 row blocks of ab (8 warps) and of cd
+template <int NT_CD>
+md4_status launch_small(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
+    if (a.wpc + 1 <= 4) return launch_one<NT_CD, 8, 4, false, 3>(ctx, a, st);
+    if (a.wpc + 1 <= 8) return launch_one<NT_CD, 8, 8, false, 2>(ctx, a, st);
+    return launch_w<NT_CD, false>(ctx, a, st);
 }
 
 }  // namespace
@@ -449,9 +463,9 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     if (nt == 16) return launch_w<16, true>(ctx, a, st);
     if (nt == 18) return launch_w<18, true>(ctx, a, st);
     if (nt == 22) return launch_w<22, true>(ctx, a, st);
-    if (nt <= 2) return launch_w<2, false>(ctx, a, st);
-    if (nt <= 4) return launch_w<4, false>(ctx, a, st);
-    if (nt <= 7) return launch_w<7, false>(ctx, a, st);
+    if (nt <= 2) return launch_small<2>(ctx, a, st);
+    if (nt <= 4) return launch_small<4>(ctx, a, st);
+    if (nt <= 7) return launch_small<7>(ctx, a, st);
     if (nt <= 12) return launch_w<12, false>(ctx, a, st);
     ctx->err = "md4_compute: ket class too large";
     return MD4_EUNSUPPORTED;

@@ -47,7 +47,7 @@ constexpr int RS2 = 631;
 __host__ __device__ inline int r_addr(int t, int u, int v) { return t * RS2 + u * RS1 + v; }
 __host__ __device__ inline int r_alloc(int L) { return L * RS2 + 32; }  // doubles; +32: padding columns read addresses 0..15 past the largest p~
 constexpr int LPAIR = 2 * LMAX;          // highest l_a + l_b of a shell pair
-constexpr int TACC_WARPS = 11;            // consumer warps per CTA of the fused kernel, at most
+constexpr int TACC_WARPS = 22;            // consumer warps per SM of the fused kernel, at most (11 per CTA; small classes: 3 CTAs x 3, 2 x 7)
 constexpr int TACC_QBLOCKS = 64;         // q~ column blocks, at most (57 for l_pair = 12)
 constexpr uint32_t COL_PAD = 1u << 31;   // flag of a padding column in the column tables
 
