@@ -193,7 +193,7 @@ def whole_job_rate(world: int, quartets_per_rank: int, ms_per_step: float) -> fl
 
 
 # ncu --set full capture of the dominant kernel (profiles/r1_eri_kernel_ncu.md): dram read + write bytes per launch
-NCU_TRAFFIC_BYTES = {"cfg3": 12.69e9}
+NCU_TRAFFIC_BYTES = {"cfg3": 12.64e9}
 
 
 def run_gpu(args):
