@@ -31,6 +31,12 @@ namespace md4 {
 namespace {
 
 constexpr int MAX_STAGES = 16;
+#ifndef PF_SMALL
+#define PF_SMALL 6
+#endif
+#ifndef PF_LARGE
+#define PF_LARGE 2
+#endif
 
 struct EriArgs {
     const double* Hb; const double* sb; const double* pmb; size_t hsb;
@@ -123,13 +129,24 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
         aqr[n] = c.ra32 + ((!PRED || n < nq) ? lds_u32(c.aq32 + (uint32_t)(j0 + n) * 32u) : 0u);
     }
     // ---- GEMM1: the B operand is G[p~,q~] = +-R[p~+q~] read at address(p~) + address(q~) (Eq.8)
-    double2 a0 = ldg2(c.Ablk);
-    double2 a1 = c.ncb_p > 1 ? ldg2(c.Ablk + c.astride) : make_double2(0.0, 0.0);
+    // H_ab fragments come from L2 (~1 us), PF k-blocks ahead.  Measured per ket class (profiles/r1_sweep.md): 6 pays
+    // for hh / ig kets (+4 %; 2 warps per sub-partition, so a k-block passes in ~1 us), costs 7 % for gg kets (short
+    // k-loops, long prologue) and 3 % for ii kets (no registers to spare)
+    constexpr int PF = (NT_CD == 15 || NT_CD == 16) ? PF_SMALL : PF_LARGE;
+    double2 af[PF];
+#pragma unroll
+    for (int i = 0; i < PF; ++i) af[i] = i < c.ncb_p ? ldg2(c.Ablk + (size_t)i * c.astride) : make_double2(0.0, 0.0);
     int2 apn = lds_v2s32(c.ap32);
     for (int jb = 0; jb < c.ncb_p; ++jb) {
-        const double2 av = a0;
-        a0 = a1;
-        if (jb + 2 < c.ncb_p) a1 = ldg2(c.Ablk + (size_t)(jb + 2) * c.astride);
+        const double2 av = af[0];
+        if constexpr (PF == 2) {
+            af[0] = af[1];
+            if (jb + 2 < c.ncb_p) af[1] = ldg2(c.Ablk + (size_t)(jb + 2) * c.astride);
+        } else {
+#pragma unroll
+            for (int i = 0; i + 1 < PF; ++i) af[i] = af[i + 1];
+            if (jb + PF < c.ncb_p) af[PF - 1] = ldg2(c.Ablk + (size_t)(jb + PF) * c.astride);
+        }
         const int2 app = apn;
         apn = lds_v2s32(c.ap32 + (uint32_t)(jb + 1) * 32u);   // the ap array has one block of slack
         double b[NQ];
