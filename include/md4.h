@@ -119,6 +119,12 @@ double md4_flops_per_quartet(const md4_pairs* bra, const md4_pairs* ket);
 
 /* ---- stage-level access for the parity tests (S:4 test layer 3) --------------------------------- */
 
+/* How md4_compute splits the (2li+1)(2lj+1) rows of a bra class into work items of 8-row blocks, one consumer warp
+ * per block (host logic only, no device needed): out7 HOST [7] = number of items per quartet (1 or 2), first row
+ * block of item 0..2, row blocks of item 0..2.  The FP64 tensor pipe of sm_100a is per SM sub-partition, so an item
+ * of n blocks costs ceil(n/4) block-times; the split minimises their sum. */
+md4_status md4_debug_work_items(int li, int lj, int* out7);
+
 /* Boys function F_m(T), m = 0..mmax (mmax <= 4*MD4_LMAX), evaluated on the device by the same device
  * function the compute kernel uses (table + Taylor, asymptotic above T_max).
  *   T HOST [n], out HOST [n*(mmax+1)] */

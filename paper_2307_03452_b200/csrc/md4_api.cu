@@ -371,6 +371,13 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
     return MD4_OK;
 }
 
+md4_status md4_debug_work_items(int li, int lj, int* out7) {
+    if (li < 0 || lj < 0 || li > LMAX || lj > LMAX || !out7) return MD4_EINVAL;
+    const int nrb = (n_solid(li) * n_solid(lj) + 7) / 8;
+    plan_items_host(nrb, out7, out7 + 1, out7 + 4);
+    return MD4_OK;
+}
+
 md4_status md4_debug_boys(md4_ctx* ctx, int mmax, int n, const double* T, double* out) {
     if (!ctx) return MD4_EINVAL;
     if (mmax < 0 || mmax > LTOT || n < 0 || (n > 0 && (!T || !out))) return fail(ctx, MD4_EINVAL, "md4_debug_boys: bad argument");

@@ -454,6 +454,14 @@ md4_status launch_small(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
 
 }  // namespace
 
+void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows) {
+    EriArgs a;
+    a.nrb_ab = nrb_ab;
+    plan_items(a);
+    *nitems = a.ncta_per_q;
+    for (int t = 0; t < 3; ++t) { row0[t] = a.row0[t]; nrows[t] = a.nrows[t]; }
+}
+
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
                       cudaStream_t st) {
     EriArgs a;

@@ -139,6 +139,7 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
 // md4_eri.cu
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
                       cudaStream_t st);
+void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows);   // the work-item split of md4_compute (host logic)
 cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, double* d_out);
 cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out);
 }  // namespace md4

@@ -22,7 +22,7 @@ SYMBOLS = [
     "md4_create", "md4_destroy", "md4_last_error", "md4_set_shells", "md4_build_pairs", "md4_free_pairs",
     "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host",
     "md4_launch_count", "md4_flops_per_quartet", "md4_debug_boys", "md4_debug_solid_coeff",
-    "md4_debug_hermite_r", "md4_debug_pair_h",
+    "md4_debug_hermite_r", "md4_debug_pair_h", "md4_debug_work_items",
 ]
 
 _lib = None
@@ -78,8 +78,20 @@ def load():
     lib.md4_debug_hermite_r.restype = ctypes.c_int
     lib.md4_debug_pair_h.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, dp, dp]
     lib.md4_debug_pair_h.restype = ctypes.c_int
+    lib.md4_debug_work_items.argtypes = [ctypes.c_int, ctypes.c_int, ip]
+    lib.md4_debug_work_items.restype = ctypes.c_int
     _lib = lib
     return lib
+
+
+def work_items(li: int, lj: int):
+    """(number of items, first row block per item, row blocks per item) of a bra class; host logic, no GPU."""
+    out = (ctypes.c_int * 7)()
+    st = load().md4_debug_work_items(li, lj, out)
+    if st != 0:
+        raise Md4Error(st, "md4_debug_work_items")
+    n = out[0]
+    return n, list(out[1:1 + n]), list(out[4:4 + n])
 
 
 def _dp(a):
