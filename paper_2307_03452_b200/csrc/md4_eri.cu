@@ -378,8 +378,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
 #pragma unroll
                     for (int nb = 0; nb < NT_CD; ++nb) {
                         const int col = nb * 8 + 2 * cc.k4;
-                        if (col < a.ncd) o[col] = (acc[nb].x * f) * f;
-                        if (col + 1 < a.ncd) o[col + 1] = (acc[nb].y * f) * f;
+                        if (col < a.ncd) __stcs(o + col, (acc[nb].x * f) * f);   // streaming store: the output must not evict H from L2
+                        if (col + 1 < a.ncd) __stcs(o + col + 1, (acc[nb].y * f) * f);
                     }
                 }
             }
