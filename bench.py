@@ -66,6 +66,49 @@ def workload_by_name(name: str, rank: int = 0):
     return wl
 
 
+def workloads_by_name(name: str, rank: int = 0):
+    """The batches of one step: one workload for cfg1-cfg4, the 42 of BASELINE.json config 5 (21 classes x K = 1, 3
+    per shell) for cfg5."""
+    if name == "cfg5":
+        return [inputs.config5(ci, K=K, seed_offset=100 * rank) for K in (1, 3) for ci in range(len(inputs.sweep_classes()))]
+    return [workload_by_name(name, rank)]
+
+
+def config_dict(wls, world: int) -> dict:
+    """The `config` object of the JSON line; both arms (ours and --impl reference) print exactly this."""
+    l2 = "no flush: inputs+outputs of a step exceed the 126 MB L2 (cfg3: H matrices 330 MB, output 3.74 GB)"
+    if len(wls) == 1:
+        wl = wls[0]
+        if wl.nquartets * inputs.class_out_doubles(wl.lclass) * 8 < (126 << 20):
+            l2 = "no flush: the pair lists are rebuilt (rewritten) every step; the output of this small batch fits L2"
+        return {"workload": wl.name, "quartets_per_gpu": wl.nquartets, "lclass": list(wl.lclass), "kclass": list(wl.kclass),
+                "seed": wl.seed, "parallelism": f"independent batches x{world}", "l2": l2}
+    return {"workload": f"cfg5 mixed-class sweep: {len(wls)} batches = 21 classes (l in 4..6) x K = 1, 3 per shell, 64 x 64 quartets each",
+            "quartets_per_gpu": sum(w.nquartets for w in wls), "lclass": None, "kclass": None, "seed": wls[0].seed,
+            "parallelism": f"independent batches x{world}", "l2": l2}
+
+
+def ncu_traffic(workload: str):
+    """dram read+write bytes per launch of the dominant kernel from the committed ncu capture, keyed by the hash of
+    the kernel sources it was taken on (profiles/traffic.json).  None (plus the reason) when the library that runs now
+    was built from other sources: a figure from another build is never reported."""
+    from paper_2307_03452_b200 import build as md4_build
+
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        tab = json.load(open(path))
+    except Exception as e:
+        return None, f"profiles/traffic.json unreadable: {e}"
+    h = md4_build.source_hash()
+    ent = tab.get("captures", {}).get(h)
+    if ent is None:
+        return None, f"no ncu capture for source hash {h} (captures: {sorted(tab.get('captures', {}))})"
+    w = ent.get(workload)
+    if w is None:
+        return None, f"capture {h} has no entry for {workload}"
+    return float(w["dram_bytes_read"]) + float(w["dram_bytes_write"]), f"profiles/traffic.json[{h}][{workload}] ({ent.get('source', '')})"
+
+
 class ClockSampler:
     """nvidia-smi clocks line of B200_PROFILING.md, sampled every 200 ms while the timed region runs."""
 
@@ -122,25 +165,46 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------ oracle leg
 def oracle_sample_rate(wl, budget_s: float = 15.0, seed: int = 12345):
     """Times the oracle as it stands (its long-double build, the precision BASELINE.json names; the binary128
-    build the parity tests use is ~8x slower) on a seeded sample of wl's quartets, all host cores, one thread
-    per quartet.  Returns (quartets/s, cores, n_sampled, seconds)."""
+    build the parity tests use is ~8x slower) on a seeded sample of wl's quartets on all host cores: one thread per
+    quartet for uncontracted classes, the primitive loop of one quartet at a time spread over the threads for
+    contracted ones.  Returns (quartets/s, cores, n_sampled, seconds)."""
     import oracle
 
     cores = os.cpu_count() or 1
     sh = oracle.Shells(wl.shells.centers, wl.shells.l, wl.shells.prim_offset, wl.shells.exponents,
                        wl.shells.coefficients)
     rng = np.random.Generator(np.random.PCG64(seed))
-    probe = rng.choice(wl.nquartets, size=min(cores, wl.nquartets), replace=False).astype(np.int32)
+    contracted = int(np.prod(wl.kclass)) >= cores
+    nslice = cores if contracted else 1
+    n0 = 1 if contracted else min(cores, wl.nquartets)
+    probe = rng.choice(wl.nquartets, size=n0, replace=False).astype(np.int32)
     t0 = time.perf_counter()
-    oracle.compute(sh, wl.bra_ij, wl.ket_ij, subset=probe, nthreads=cores, precision="ld")
+    oracle.compute(sh, wl.bra_ij, wl.ket_ij, subset=probe, nthreads=cores, precision="ld", nslice=nslice)
     t_probe = max(time.perf_counter() - t0, 1e-6)
-    n = int(max(cores, min(wl.nquartets, (budget_s / t_probe) * len(probe))))
-    n = min(n, wl.nquartets)
+    n = int(max(n0, min(wl.nquartets, (budget_s / t_probe) * n0)))
+    if n == n0:
+        return n0 / t_probe, cores, n0, t_probe
     sub = rng.choice(wl.nquartets, size=n, replace=False).astype(np.int32)
     t0 = time.perf_counter()
-    oracle.compute(sh, wl.bra_ij, wl.ket_ij, subset=sub, nthreads=cores, precision="ld")
+    oracle.compute(sh, wl.bra_ij, wl.ket_ij, subset=sub, nthreads=cores, precision="ld", nslice=nslice)
     dt = time.perf_counter() - t0
     return n / dt, cores, n, dt
+
+
+def oracle_step(wls, budget_s: float):
+    """One bounded oracle pass over the batches of a step.  Returns (whole-step quartets/s = total quartets / sum over
+    batches of quartets_b / rate_b, cores, quartets sampled, seconds spent)."""
+    t_full, nsamp, spent, cores = 0.0, 0, 0.0, 1
+    for wl in wls:
+        r, cores, n, dt = oracle_sample_rate(wl, budget_s=budget_s / len(wls))
+        t_full += wl.nquartets / r
+        nsamp += n
+        spent += dt
+    return sum(w.nquartets for w in wls) / t_full, cores, nsamp, spent
+
+
+def total_flops(wls) -> float:
+    return float(sum(w.nquartets * inputs.class_flops(w.lclass, w.kclass) for w in wls))
 
 
 def run_reference(args):
@@ -148,25 +212,26 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    wl = workload_by_name(args.workload)
+    wls = workloads_by_name(args.workload)
+    nq = sum(w.nquartets for w in wls)
     per_step_budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
-        oracle_sample_rate(wl, budget_s=per_step_budget)
+        oracle_step(wls, per_step_budget)
     rates, ns, secs, cores = [], [], [], 1
     for _ in range(args.steps):
-        r, cores, n, dt = oracle_sample_rate(wl, budget_s=per_step_budget)
+        r, cores, n, dt = oracle_step(wls, per_step_budget)
         rates.append(r); ns.append(n); secs.append(dt)
-    value = sum(ns) / sum(secs)
-    flops = inputs.class_flops(wl.lclass, wl.kclass)
-    sample = f"{ns[0]} seeded random quartets of {wl.nquartets} per step, {cores} threads (one quartet per thread at a time)"
+    value = len(rates) / sum(1.0 / r for r in rates)     # harmonic mean = total quartets / total (extrapolated) time
+    sample = (f"{ns[0]} seeded random quartets of {nq} per step in {secs[0]:.1f} s, {cores} threads; step rate = total quartets / "
+              f"sum over batches of (quartets / sampled rate)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / len(secs), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
-        "config": {"workload": wl.name, "quartets": wl.nquartets, "lclass": list(wl.lclass), "kclass": list(wl.kclass),
-                   "seed": wl.seed},
-        "tflops": value * flops / 1e12,
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle (long-double build)", "sample": sample},
+        "config": config_dict(wls, max(1, args.gpus)),
+        "tflops": value * total_flops(wls) / nq / 1e12,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle (long-double build, as it stands: not a tuned CPU code)",
+                         "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -192,10 +257,6 @@ def whole_job_rate(world: int, quartets_per_rank: int, ms_per_step: float) -> fl
     return world * quartets_per_rank / (ms_per_step * 1e-3)
 
 
-# ncu --set full capture of the dominant kernel (profiles/r1_eri_kernel_ncu.md): dram read + write bytes per launch
-NCU_TRAFFIC_BYTES = {"cfg3": 12.64e9}
-
-
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -209,10 +270,7 @@ def run_gpu(args):
     if local == 0:
         md4_build.ensure_built()   # a checkout has no build artefacts; the kernels themselves have no fallback
     else:
-        for _ in range(600):       # the other local ranks wait for rank 0's build
-            if os.path.exists(md4_build.LIB):
-                break
-            time.sleep(0.5)
+        md4_build.wait_until_built()   # the other local ranks wait for rank 0's build (atomic rename, never a partial file)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the MD4 path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -224,35 +282,47 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = workload_by_name(args.workload, rank)
-    s = wl.shells
+    wls = workloads_by_name(args.workload, rank)
+    multi = len(wls) > 1
     eng = md4.Engine(local)
-    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
     stream = torch.cuda.current_stream()
-    nq = wl.nquartets
-    flops_q = inputs.class_flops(wl.lclass, wl.kclass)
-    out_doubles = nq * inputs.class_out_doubles(wl.lclass)
-    out = torch.empty(out_doubles, dtype=torch.float64, device=f"cuda:{local}")
+    nq = sum(w.nquartets for w in wls)
+    flops_step = total_flops(wls)
+    out_doubles = [w.nquartets * inputs.class_out_doubles(w.lclass) for w in wls]
+    out = torch.empty(max(out_doubles), dtype=torch.float64, device=f"cuda:{local}")
 
-    kern_ev = []
+    def upload(wl):
+        s = wl.shells
+        eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+
+    if not multi:
+        upload(wls[0])            # shells resident in HBM before the timed region; cfg5 changes the shell set per class
+    kern_ev = [[] for _ in wls]
     prev = []
 
     def step(timed: bool):
-        # the lists of the step before are released first (md4_free_pairs waits for the work that reads them and
-        # hands their buffers to the next md4_build_pairs): the loop a user of the library would write
+        # the lists of the step before are released first (md4_free_pairs hands their memory, with the event of the
+        # launch that still reads it, to the next md4_build_pairs): the loop a user of the library would write.
+        # Nothing in a step blocks the host: copies, pair kernels and the fused kernel are stream-ordered.
         while prev:
             b, k = prev.pop()
             b.free(); k.free()
-        bra = eng.build_pairs(wl.bra_ij)
-        ket = eng.build_pairs(wl.ket_ij)
-        if timed:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-        eng.compute(bra, ket, out=out, stream=stream.cuda_stream)
-        if timed:
-            e1.record(stream)
-            kern_ev.append((e0, e1))
-        prev.append((bra, ket))
+        for w, wl in enumerate(wls):
+            if multi:
+                upload(wl)
+            bra = eng.build_pairs(wl.bra_ij)
+            ket = eng.build_pairs(wl.ket_ij)
+            if timed:
+                # the kernel's own duration: the events go behind the (device-side) wait for the two pair kernels
+                eng.stream_wait_pairs(bra, stream.cuda_stream)
+                eng.stream_wait_pairs(ket, stream.cuda_stream)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+            eng.compute(bra, ket, out=out, stream=stream.cuda_stream)
+            if timed:
+                e1.record(stream)
+                kern_ev[w].append((e0, e1))
+            prev.append((bra, ket))
 
     # ---- device-resident arm: W warm-up steps, then exactly K timed steps
     for _ in range(args.warmup):
@@ -275,23 +345,24 @@ def run_gpu(args):
         b, k = prev.pop()
         b.free(); k.free()
     ms_total = reduce_max(t0.elapsed_time(t1), world, f"cuda:{local}")
-    kern_ms = [a.elapsed_time(b) for a, b in kern_ev]
+    kern_ms = [statistics.mean(a.elapsed_time(b) for a, b in evs) for evs in kern_ev]
     ms_step = ms_total / args.steps
     value = whole_job_rate(world, nq, ms_step)
 
     # ---- end-to-end arm through HOST buffers (same K steps; H2D of shells + pair lists, D2H of all integrals)
-    host = torch.empty(out_doubles, dtype=torch.float64, pin_memory=True)
+    host = torch.empty(max(out_doubles), dtype=torch.float64, pin_memory=True)
     host_np = host.numpy()
-    h2d = int(s.centers.nbytes + s.l.nbytes + s.prim_offset.nbytes + s.exponents.nbytes + s.coefficients.nbytes +
-              wl.bra_ij.nbytes + wl.ket_ij.nbytes)
-    d2h = int(out_doubles * 8)
+    h2d = int(sum(w.shells.centers.nbytes + w.shells.l.nbytes + w.shells.prim_offset.nbytes + w.shells.exponents.nbytes +
+                  w.shells.coefficients.nbytes + w.bra_ij.nbytes + w.ket_ij.nbytes for w in wls))
+    d2h = int(sum(out_doubles) * 8)
 
     def e2e_step():
-        eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
-        bra = eng.build_pairs(wl.bra_ij)
-        ket = eng.build_pairs(wl.ket_ij)
-        eng.compute_host(bra, ket, out=host_np, stream=stream.cuda_stream)
-        bra.free(); ket.free()
+        for wl in wls:
+            upload(wl)
+            bra = eng.build_pairs(wl.bra_ij)
+            ket = eng.build_pairs(wl.ket_ij)
+            eng.compute_host(bra, ket, out=host_np, stream=stream.cuda_stream)
+            bra.free(); ket.free()
 
     e2e_step()
     barrier()
@@ -304,28 +375,36 @@ def run_gpu(args):
 
     if rank == 0:
         peak, peak_how = fp64_peak_tflops()
-        k_ms = statistics.mean(kern_ms)
-        achieved = nq * flops_q / (k_ms * 1e-3) / 1e12
+        traffic, traffic_src = ncu_traffic(args.workload)
+        k_ms = sum(kern_ms)
+        achieved = flops_step / (k_ms * 1e-3) / 1e12
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": wl.name, "quartets_per_gpu": nq, "lclass": list(wl.lclass), "kclass": list(wl.kclass),
-                       "seed": wl.seed, "parallelism": f"independent batches x{world}",
-                       "l2": "inputs+outputs larger than L2 (H matrices 157 MB, output 3.74 GB for cfg3); no flush"},
-            "tflops": value * flops_q / 1e12, "fp64_peak_frac": value * flops_q / 1e12 / (peak * world),
-            "flops_per_quartet": flops_q,
+            "config": config_dict(wls, world),
+            "tflops": value * flops_step / nq / 1e12, "fp64_peak_frac": value * flops_step / nq / 1e12 / (peak * world),
+            "flops_per_quartet": flops_step / nq,
             "roofline": {"bound": "tensor", "kernel": "md4::eri_kernel (FP64 DMMA.8x8x4)", "achieved": achieved,
-                         "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-                         "traffic_unit": "bytes per launch (dram read+write, profiles/r1_eri_kernel_ncu.md)",
-                         "algorithmic_bytes": out_doubles * 8,
+                         "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                         "traffic_unit": "bytes per launch (dram read+write)", "traffic_source": traffic_src,
+                         "algorithmic_bytes": int(sum(out_doubles) * 8),
                          "peak_source": peak_how, "kernel_ms": k_ms},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(n_launch), "clocks": clocks,
         }
+        if multi:
+            # BASELINE.json config 5: per-class quartets/s and % of FP64 peak (fused kernel alone, CUDA events)
+            line["classes"] = [
+                {"name": w.name, "lclass": list(w.lclass), "kclass": list(w.kclass), "quartets": w.nquartets,
+                 "kernel_ms": ms, "quartets_per_s": w.nquartets / (ms * 1e-3),
+                 "tflops": w.nquartets * inputs.class_flops(w.lclass, w.kclass) / (ms * 1e-3) / 1e12,
+                 "frac": w.nquartets * inputs.class_flops(w.lclass, w.kclass) / (ms * 1e-3) / 1e12 / peak}
+                for w, ms in zip(wls, kern_ms)]
         if world == 1 and not args.no_cpu_baseline:
-            r, cores, n, dt = oracle_sample_rate(wl, budget_s=15.0)
-            line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle (long-double build)",
+            r, cores, n, dt = oracle_step(wls, 15.0)
+            line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores,
+                                    "kind": "oracle (long-double build, as it stands: not a tuned CPU code)",
                                     "sample": f"{n} seeded random quartets of {nq} in {dt:.1f} s, {cores} threads"}
         print(json.dumps(line), flush=True)
     eng.close()
@@ -339,7 +418,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

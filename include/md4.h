@@ -21,7 +21,15 @@
  * caller may free them on return.  The output buffer is a caller-owned DEVICE buffer.
  * Errors: every entry point returns md4_status (or writes nothing and returns NULL/void where noted);
  * nothing throws or aborts across the ABI.  md4_last_error() gives a human-readable reason.
- * Threading: a context is not thread-safe; distinct contexts are independent.
+ * Threading: a context is not thread-safe (one host thread at a time); distinct contexts are independent.
+ * Stream ordering: no entry point except md4_compute_host, md4_destroy and the md4_debug_* calls waits for
+ * the device.  md4_set_shells and md4_build_pairs enqueue their copies and the pair kernel on an internal
+ * stream of the context; md4_compute makes the caller's stream wait (on the device) for the pair kernels of
+ * both lists.  md4_compute may be called on several streams of one context: launches whose bra list is
+ * contracted share one scratch buffer of the context and are therefore ordered one after the other by an
+ * internal event (each launch is a persistent grid that fills the GPU, so nothing is lost); all other
+ * launches are independent.  md4_free_pairs never synchronises: the list's memory is handed to the next
+ * md4_build_pairs together with the event of its last reader.
  */
 #ifndef MD4_H
 #define MD4_H
@@ -76,11 +84,20 @@ md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, c
  * = c_ka c_kb * C_la (x) C_lb * E, on the device.  All pairs must share (l_i, l_j, K_i, K_j), else
  * MD4_EINVAL.  A list is role-agnostic: the same list may serve as bra and as ket.
  *   ij   HOST [npair*2]  shell indices (i0,j0,i1,j1,...)
- * npair == 0 gives a valid empty list.  *out is NULL on failure. */
+ * npair == 0 gives a valid empty list.  *out is NULL on failure.  The call validates, copies ij and
+ * enqueues the pair kernel on the context's internal stream; it does not wait for the kernel (it blocks only
+ * when it is several builds ahead of the device).  Device memory comes from the context's pool of released
+ * lists when a block of about that size is there (at most 4 GB are kept idle; env MD4_POOL_MAX_MB). */
 md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** out);
 
-/* Release one pair list (also done by md4_destroy).  NULL is a no-op. */
+/* Release one pair list (also done by md4_destroy).  NULL is a no-op.  Does not synchronise: launches that still
+ * read the list finish first, on the device, before its memory is overwritten by a later md4_build_pairs. */
 void md4_free_pairs(md4_ctx* ctx, md4_pairs* pairs);
+
+/* Make cuda_stream wait, on the device, until the pair kernel of `pairs` has finished (the call itself returns at
+ * once).  md4_compute does this for both of its lists; the call is for a caller that orders its own work -- or its
+ * timing events, as bench.py does -- behind md4_build_pairs. */
+md4_status md4_stream_wait_pairs(md4_ctx* ctx, const md4_pairs* pairs, void* cuda_stream);
 
 /* Shape queries of a pair list; return -1 for NULL. */
 int md4_pairs_count(const md4_pairs* pairs);
@@ -97,7 +114,9 @@ md4_status md4_output_size(const md4_pairs* bra, const md4_pairs* ket, size_t* n
  *   d_out   DEVICE, 8-byte aligned, capacity_doubles >= md4_output_size; fully OVERWRITTEN with
  *           out[i_bra][j_ket][ma][mb][mc][md], row-major, md fastest, m = -l..+l ascending.
  *   cuda_stream  the caller's cudaStream_t (NULL = default stream).  The call only enqueues work on
- *           that stream and returns: no device synchronisation, no allocation.
+ *           that stream and returns: no device synchronisation, no allocation.  The stream first waits for
+ *           the pair kernels of both lists (and, for a contracted bra, for the previous such launch of this
+ *           context, see "Stream ordering" above).
  * On any error nothing is enqueued.  Empty lists: MD4_OK, nothing written. */
 md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out,
                        size_t capacity_doubles, void* cuda_stream);

@@ -27,12 +27,32 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+HASHFILE = os.path.join(OBJ, "libmd4.srchash")
+
+
+def source_hash() -> str:
+    """sha256 over the contents of every source and header of libmd4 plus the compiler flags (16 hex digits).  The
+    build records it beside the library; bench.py keys the committed ncu traffic figure on it (profiles/*.json), so a
+    figure captured on another build is never reported."""
+    import hashlib
+
+    h = hashlib.sha256()
+    for rel in sorted(SOURCES + HEADERS):
+        with open(os.path.join(CSRC, rel), "rb") as f:
+            h.update(rel.replace(os.sep, "/").encode() + b"\0" + f.read() + b"\0")
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()[:16]
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    """Content-based (file times do not survive a repository snapshot): the library is current if the hash recorded
+    when it was linked equals the hash of the sources now."""
+    if not os.path.exists(LIB) or not os.path.exists(HASHFILE):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    try:
+        return open(HASHFILE).read().strip() != source_hash()
+    except OSError:
+        return True
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -55,16 +75,40 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
-    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+    # link under a temporary name and rename: a process that finds libmd4.so never sees a half-written file
+    tmp = f"{LIB}.{os.getpid()}.tmp"
+    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
+        if os.path.exists(tmp):
+            os.unlink(tmp)
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    if os.path.exists(HASHFILE):
+        os.unlink(HASHFILE)
+    os.replace(tmp, LIB)
+    with open(HASHFILE + ".tmp", "w") as f:
+        f.write(source_hash() + "\n")
+    os.replace(HASHFILE + ".tmp", HASHFILE)
     return LIB
 
 
 def ensure_built() -> str:
-    """Compile libmd4.so if it is not there (a checkout without build artefacts); never a fallback for the kernels."""
-    return LIB if os.path.exists(LIB) else build(force=True)
+    """Compile libmd4.so if it is missing or older than its sources (a checkout has no build artefacts; an edited
+    csrc/ must never run as a stale binary); never a fallback for the kernels."""
+    return build()
+
+
+def wait_until_built(timeout_s: float = 600.0) -> str:
+    """For the local ranks > 0 of a multi-process launch: wait until rank 0's ensure_built() has left a library that is
+    newer than every source (the rename in build() makes its appearance atomic)."""
+    import time
+
+    t0 = time.time()
+    while _stale():
+        if time.time() - t0 > timeout_s:
+            raise RuntimeError("libmd4.so was not built in time by local rank 0")
+        time.sleep(0.25)
+    return LIB
 
 
 if __name__ == "__main__":

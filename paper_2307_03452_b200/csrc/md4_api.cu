@@ -1,6 +1,7 @@
 // md4_api.cu -- the C ABI of include/md4.h: context, shells, pair lists, compute dispatch.
 // Host logic only; every step of the hot path runs in the kernels of md4_pairs.cu / md4_eri.cu.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -30,59 +31,82 @@ md4_status cuda_fail(md4_ctx* ctx, const char* what, cudaError_t e) {
     return fail(ctx, e == cudaErrorMemoryAllocation ? MD4_ENOMEM : MD4_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 
-void free_shells(md4_ctx* c) {
-    cudaFree(c->d_centers); cudaFree(c->d_l); cudaFree(c->d_off); cudaFree(c->d_exp); cudaFree(c->d_coef);
+// forget the shell set (the device block is kept for the next one); release: the context is going away
+void free_shells(md4_ctx* c, bool release = false) {
     c->d_centers = nullptr; c->d_l = nullptr; c->d_off = nullptr; c->d_exp = nullptr; c->d_coef = nullptr;
     c->nshell = 0; c->nprim = 0; c->h_l.clear(); c->h_off.clear();
+    if (release) {
+        cudaFree(c->d_shell_block); c->d_shell_block = nullptr; c->shell_block_bytes = 0;
+        if (c->h_shell_stage) cudaFreeHost(c->h_shell_stage);
+        c->h_shell_stage = nullptr; c->shell_stage_bytes = 0;
+        if (c->shell_done) cudaEventDestroy(c->shell_done);
+        c->shell_done = nullptr;
+    }
 }
 
-// ---- pool of H buffers ------------------------------------------------------------------------------
-constexpr size_t POOL_MIN_BYTES = (size_t)1 << 20;    // smaller blocks go straight to cudaMalloc/cudaFree
-constexpr size_t POOL_MAX_BYTES = (size_t)16 << 30;   // bytes kept idle at most
+// ---- pool of pair-list blocks --------------------------------------------------------------------------
+// A released list's block goes here together with the event of its last reader; the next md4_build_pairs of about
+// that size takes it and makes its pair kernel wait for that event on the device.  Nothing here blocks the host.
+constexpr size_t POOL_MIN_BYTES = (size_t)64 << 10;          // smaller blocks go straight to cudaMalloc/cudaFree
+constexpr size_t POOL_MAX_DEFAULT = (size_t)4 << 30;         // bytes kept idle at most (env MD4_POOL_MAX_MB overrides)
 
-cudaError_t pool_alloc(md4_ctx* c, size_t bytes, double** out) {
-    *out = nullptr;
-    if (bytes >= POOL_MIN_BYTES) {
-        auto it = c->pool.lower_bound(bytes);
-        if (it != c->pool.end() && it->first <= bytes + bytes / 4) {
-            *out = static_cast<double*>(it->second);
-            c->pool_bytes -= it->first;
-            c->pool.erase(it);
-            return cudaSuccess;
-        }
+void pool_release(md4_ctx* c) {
+    for (auto& kv : c->pool) {
+        if (kv.second.ev) { cudaEventSynchronize(kv.second.ev); cudaEventDestroy(kv.second.ev); }
+        cudaFree(kv.second.p);
     }
-    cudaError_t e = cudaMalloc((void**)out, bytes ? bytes : 8);
+    c->pool.clear(); c->pool_bytes = 0;
+}
+
+// cudaMalloc for anything the context owns: on out-of-memory the idle pool is released and the call retried once
+cudaError_t ctx_malloc(md4_ctx* c, void** out, size_t bytes) {
+    *out = nullptr;
+    cudaError_t e = cudaMalloc(out, bytes ? bytes : 8);
     if (e == cudaErrorMemoryAllocation && !c->pool.empty()) {
         (void)cudaGetLastError();
-        for (auto& kv : c->pool) cudaFree(kv.second);
-        c->pool.clear(); c->pool_bytes = 0;
-        e = cudaMalloc((void**)out, bytes ? bytes : 8);
+        pool_release(c);
+        e = cudaMalloc(out, bytes ? bytes : 8);
     }
     return e;
 }
 
-void pool_free(md4_ctx* c, void* p, size_t bytes) {
-    if (!p) return;
-    if (c && bytes >= POOL_MIN_BYTES && c->pool_bytes + bytes <= POOL_MAX_BYTES) {
-        c->pool.emplace(bytes, p);
-        c->pool_bytes += bytes;
+cudaError_t pool_alloc(md4_ctx* c, size_t bytes, PoolBlock* out) {
+    *out = PoolBlock();
+    if (bytes >= POOL_MIN_BYTES) {
+        auto it = c->pool.lower_bound(bytes);
+        if (it != c->pool.end() && it->first <= bytes + bytes / 4) {
+            *out = it->second;
+            c->pool_bytes -= it->second.bytes;
+            c->pool.erase(it);
+            return cudaSuccess;
+        }
+    }
+    cudaError_t e = ctx_malloc(c, &out->p, bytes);
+    if (e == cudaSuccess) out->bytes = bytes ? bytes : 8;
+    return e;
+}
+
+// c == nullptr: the context is going away (everything has been synchronised), free for real
+void pool_free(md4_ctx* c, PoolBlock blk) {
+    if (!blk.p) { if (blk.ev) cudaEventDestroy(blk.ev); return; }
+    if (c && blk.bytes >= POOL_MIN_BYTES && c->pool_bytes + blk.bytes <= c->pool_max_bytes) {
+        c->pool.emplace(blk.bytes, blk);
+        c->pool_bytes += blk.bytes;
     } else {
-        cudaFree(p);
+        if (blk.ev) { cudaEventSynchronize(blk.ev); cudaEventDestroy(blk.ev); }
+        cudaFree(blk.p);
     }
 }
 
-void pool_release(md4_ctx* c) {
-    for (auto& kv : c->pool) cudaFree(kv.second);
-    c->pool.clear(); c->pool_bytes = 0;
-}
-
-// to_pool: the list's work on the device is known to be complete, its H buffers may be reused
+// to_pool: the block may be handed to the next list (with the event of its last reader)
 void free_pair_storage(md4_pairs* p, bool to_pool) {
-    const size_t nprim = (size_t)p->d.npair * p->d.Ki * p->d.Kj;
-    md4_ctx* c = to_pool ? p->ctx : nullptr;
-    pool_free(c, p->d.Hb, nprim * p->d.hstrideb * sizeof(double));
-    pool_free(c, p->d.Hk, nprim * p->d.hstridek * sizeof(double));
-    cudaFree(p->d.scal); cudaFree(p->d.pairmax); cudaFree(p->d.ij);
+    PoolBlock blk = p->block;
+    // the block is free once the list's own pair kernel and its last reader are done; both events are recorded in
+    // stream order after each other's work only if a compute ran, so keep the later one: last_use if used, else ready
+    blk.ev = p->used ? p->last_use : p->ready;
+    cudaEvent_t other = p->used ? p->ready : p->last_use;
+    if (other) cudaEventDestroy(other);
+    pool_free(to_pool ? p->ctx : nullptr, blk);
     delete p;
 }
 
@@ -145,9 +169,18 @@ md4_status md4_create(md4_ctx** out, int cuda_device) {
         e = cudaMalloc(&t, (size_t)c->num_sms * TACC_WARPS * TACC_QBLOCKS * 64 * sizeof(double));
         if (e == cudaSuccess) { c->table_allocs.push_back(t); c->d_tacc = static_cast<double*>(t); }
     }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->build_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->tacc_free, cudaEventDisableTiming);
+    c->pool_max_bytes = POOL_MAX_DEFAULT;
+    if (const char* env = std::getenv("MD4_POOL_MAX_MB")) {
+        const long long mb = std::atoll(env);
+        if (mb >= 0) c->pool_max_bytes = (size_t)mb << 20;
+    }
     if (e != cudaSuccess) {
         g_create_err = std::string("md4_create: table upload: ") + cudaGetErrorString(e);
         for (void* p : c->table_allocs) cudaFree(p);
+        if (c->build_stream) cudaStreamDestroy(c->build_stream);
+        if (c->tacc_free) cudaEventDestroy(c->tacc_free);
         delete c;
         return e == cudaErrorMemoryAllocation ? MD4_ENOMEM : MD4_ECUDA;
     }
@@ -162,13 +195,19 @@ void md4_destroy(md4_ctx* ctx) {
     for (md4_pairs* p : ctx->lists) free_pair_storage(p, false);
     ctx->lists.clear();
     pool_release(ctx);
-    free_shells(ctx);
+    free_shells(ctx, true);
     cudaFree(ctx->d_scratch);
     if (ctx->copy_stream) {
         for (int i = 0; i < md4_ctx::NSLICE_EV; ++i) cudaEventDestroy(ctx->slice_ev[i]);
         cudaStreamDestroy(ctx->copy_stream);
     }
     for (void* p : ctx->table_allocs) cudaFree(p);
+    if (ctx->build_stream) cudaStreamDestroy(ctx->build_stream);
+    if (ctx->tacc_free) cudaEventDestroy(ctx->tacc_free);
+    for (int i = 0; i < md4_ctx::NSTAGE; ++i) {
+        if (ctx->stage_done[i]) cudaEventDestroy(ctx->stage_done[i]);
+        if (ctx->h_stage[i]) cudaFreeHost(ctx->h_stage[i]);
+    }
     delete ctx;
 }
 
@@ -199,12 +238,43 @@ md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, c
     DeviceGuard g(ctx->device);
     free_shells(ctx);
     if (nshell == 0) return MD4_OK;
-    cudaError_t e = upload<double>(nullptr, centers_xyz, (size_t)nshell * 3, &ctx->d_centers);
-    if (e == cudaSuccess) e = upload<int>(nullptr, l, nshell, &ctx->d_l);
-    if (e == cudaSuccess) e = upload<int>(nullptr, prim_offset, (size_t)nshell + 1, &ctx->d_off);
-    if (e == cudaSuccess) e = upload<double>(nullptr, exponents, nprim, &ctx->d_exp);
-    if (e == cudaSuccess) e = upload<double>(nullptr, coefficients, nprim, &ctx->d_coef);
-    if (e != cudaSuccess) { free_shells(ctx); return cuda_fail(ctx, "md4_set_shells", e); }
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    const size_t oC = 0, oE = oC + up((size_t)nshell * 3 * sizeof(double)), oK = oE + up((size_t)nprim * sizeof(double)),
+                 oL = oK + up((size_t)nprim * sizeof(double)), oO = oL + up((size_t)nshell * sizeof(int)),
+                 total = oO + up(((size_t)nshell + 1) * sizeof(int));
+    cudaError_t e = cudaSuccess;
+    if (!ctx->shell_done) e = cudaEventCreateWithFlags(&ctx->shell_done, cudaEventDisableTiming);
+    else e = cudaEventSynchronize(ctx->shell_done);          // the staging buffer is free again
+    if (e == cudaSuccess && ctx->shell_stage_bytes < total) {
+        if (ctx->h_shell_stage) cudaFreeHost(ctx->h_shell_stage);
+        ctx->h_shell_stage = nullptr; ctx->shell_stage_bytes = 0;
+        e = cudaMallocHost(&ctx->h_shell_stage, total);
+        if (e == cudaSuccess) ctx->shell_stage_bytes = total;
+    }
+    if (e == cudaSuccess && ctx->shell_block_bytes < total) {
+        cudaFree(ctx->d_shell_block);                         // rare (the block only grows); waits for pending pair kernels
+        ctx->d_shell_block = nullptr; ctx->shell_block_bytes = 0;
+        e = ctx_malloc(ctx, &ctx->d_shell_block, total);
+        if (e == cudaSuccess) ctx->shell_block_bytes = total;
+    }
+    if (e == cudaSuccess) {
+        char* h = static_cast<char*>(ctx->h_shell_stage);
+        std::memcpy(h + oC, centers_xyz, (size_t)nshell * 3 * sizeof(double));
+        std::memcpy(h + oE, exponents, (size_t)nprim * sizeof(double));
+        std::memcpy(h + oK, coefficients, (size_t)nprim * sizeof(double));
+        std::memcpy(h + oL, l, (size_t)nshell * sizeof(int));
+        std::memcpy(h + oO, prim_offset, ((size_t)nshell + 1) * sizeof(int));
+        // stream-ordered behind the pair kernels that still read the previous shell set
+        e = cudaMemcpyAsync(ctx->d_shell_block, h, total, cudaMemcpyHostToDevice, ctx->build_stream);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->shell_done, ctx->build_stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_set_shells", e);
+    char* dbase = static_cast<char*>(ctx->d_shell_block);
+    ctx->d_centers = reinterpret_cast<double*>(dbase + oC);
+    ctx->d_exp = reinterpret_cast<double*>(dbase + oE);
+    ctx->d_coef = reinterpret_cast<double*>(dbase + oK);
+    ctx->d_l = reinterpret_cast<int*>(dbase + oL);
+    ctx->d_off = reinterpret_cast<int*>(dbase + oO);
     ctx->nshell = nshell; ctx->nprim = nprim;
     ctx->h_l.assign(l, l + nshell);
     ctx->h_off.assign(prim_offset, prim_offset + nshell + 1);
@@ -245,16 +315,58 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
     pl->d = d;
     if (npair > 0) {
         DeviceGuard g(ctx->device);
+        // one block per list: Hb | Hk | scal | pairmax | ij (every part 256-byte aligned)
         const size_t nprim = (size_t)npair * d.Ki * d.Kj;
-        cudaError_t e = pool_alloc(ctx, nprim * d.hstrideb * sizeof(double), &pl->d.Hb);
-        if (e == cudaSuccess) e = pool_alloc(ctx, nprim * d.hstridek * sizeof(double), &pl->d.Hk);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.scal, nprim * 8 * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.pairmax, (size_t)npair * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->d.ij, (size_t)npair * 2 * sizeof(int));
-        if (e == cudaSuccess) e = cudaMemcpy(pl->d.ij, ij, (size_t)npair * 2 * sizeof(int), cudaMemcpyHostToDevice);
-        if (e == cudaSuccess) e = launch_pair_kernel(ctx, pl->d, 0);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(0);
-        if (e != cudaSuccess) { free_pair_storage(pl, false); return cuda_fail(ctx, "md4_build_pairs", e); }
+        auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+        const size_t oHb = 0, oHk = oHb + up(nprim * d.hstrideb * sizeof(double)), oSc = oHk + up(nprim * d.hstridek * sizeof(double)),
+                     oPm = oSc + up(nprim * 8 * sizeof(double)), oIj = oPm + up((size_t)npair * sizeof(double)),
+                     total = oIj + up((size_t)npair * 2 * sizeof(int));
+        cudaError_t e = pool_alloc(ctx, total, &pl->block);
+        if (e == cudaSuccess) {
+            char* base = static_cast<char*>(pl->block.p);
+            pl->d.Hb = reinterpret_cast<double*>(base + oHb);
+            pl->d.Hk = reinterpret_cast<double*>(base + oHk);
+            pl->d.scal = reinterpret_cast<double*>(base + oSc);
+            pl->d.pairmax = reinterpret_cast<double*>(base + oPm);
+            pl->d.ij = reinterpret_cast<int*>(base + oIj);
+            e = cudaEventCreateWithFlags(&pl->ready, cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->last_use, cudaEventDisableTiming);
+        // a recycled block: its previous readers finish before the pair kernel overwrites it (device-side wait)
+        if (e == cudaSuccess && pl->block.ev) {
+            e = cudaStreamWaitEvent(ctx->build_stream, pl->block.ev, 0);
+            cudaEventDestroy(pl->block.ev);
+            pl->block.ev = nullptr;
+        }
+        // ij is copied to pinned staging before the call returns (the caller may free it); transfer and kernel are only
+        // enqueued: md4_compute waits for `ready` on the device.  The host blocks only if all NSTAGE staging slots
+        // still wait for their transfers, i.e. when it is that many builds ahead of the device
+        if (e == cudaSuccess) {
+            const int sl = ctx->stage_next;
+            ctx->stage_next = (sl + 1) % md4_ctx::NSTAGE;
+            const size_t n = (size_t)npair * 2;
+            if (ctx->stage_done[sl]) e = cudaEventSynchronize(ctx->stage_done[sl]);
+            else e = cudaEventCreateWithFlags(&ctx->stage_done[sl], cudaEventDisableTiming);
+            if (e == cudaSuccess && ctx->stage_ints[sl] < n) {
+                if (ctx->h_stage[sl]) cudaFreeHost(ctx->h_stage[sl]);
+                ctx->h_stage[sl] = nullptr; ctx->stage_ints[sl] = 0;
+                const size_t cap = n < 4096 ? 4096 : n;
+                e = cudaMallocHost((void**)&ctx->h_stage[sl], cap * sizeof(int));
+                if (e == cudaSuccess) ctx->stage_ints[sl] = cap;
+            }
+            if (e == cudaSuccess) {
+                std::memcpy(ctx->h_stage[sl], ij, n * sizeof(int));
+                e = cudaMemcpyAsync(pl->d.ij, ctx->h_stage[sl], n * sizeof(int), cudaMemcpyHostToDevice, ctx->build_stream);
+            }
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->stage_done[sl], ctx->build_stream);
+        }
+        if (e == cudaSuccess) e = launch_pair_kernel(ctx, pl->d, ctx->build_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(pl->ready, ctx->build_stream);
+        if (e != cudaSuccess) {
+            cudaStreamSynchronize(ctx->build_stream);
+            free_pair_storage(pl, false);
+            return cuda_fail(ctx, "md4_build_pairs", e);
+        }
     }
     ctx->lists.insert(pl);
     *out = pl;
@@ -267,9 +379,21 @@ void md4_free_pairs(md4_ctx* ctx, md4_pairs* pairs) {
     if (it == ctx->lists.end()) return;
     ctx->lists.erase(it);
     DeviceGuard g(ctx->device);
-    // same guarantee cudaFree gave: work that still reads the list has finished before its buffers are reused
-    cudaDeviceSynchronize();
+    // no synchronisation: the block keeps the event of its last reader, and whoever gets the block next waits for it
+    // on the device (pool_alloc / md4_build_pairs); blocks too small for the pool wait for that event on the host
     free_pair_storage(pairs, true);
+}
+
+md4_status md4_stream_wait_pairs(md4_ctx* ctx, const md4_pairs* pairs, void* cuda_stream) {
+    if (!ctx) return MD4_EINVAL;
+    if (!pairs) return fail(ctx, MD4_EINVAL, "md4_stream_wait_pairs: pair list is NULL");
+    if (pairs->ctx != ctx || !ctx->lists.count(const_cast<md4_pairs*>(pairs)))
+        return fail(ctx, MD4_ESTATE, "md4_stream_wait_pairs: pair list does not belong to this context");
+    if (!pairs->ready) return MD4_OK;   // empty list: nothing was enqueued
+    DeviceGuard g(ctx->device);
+    cudaError_t e = cudaStreamWaitEvent((cudaStream_t)cuda_stream, pairs->ready, 0);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_stream_wait_pairs", e);
+    return MD4_OK;
 }
 
 int md4_pairs_count(const md4_pairs* pairs) { return pairs ? pairs->d.npair : -1; }
@@ -309,13 +433,45 @@ static md4_status check_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pa
     return MD4_OK;
 }
 
+// Stream ordering around a launch (all device-side, the host never blocks): the launch waits for the pair kernels of
+// both lists; a launch with a contracted bra also waits for the previous user of the context's [ab|q~] scratch, so
+// two md4_compute calls on different streams of one context cannot race on it (they run one after the other -- each
+// is a persistent grid that fills the GPU anyway); afterwards both lists remember the launch as their last reader.
+static cudaError_t order_before(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, cudaStream_t st) {
+    cudaError_t e = cudaStreamWaitEvent(st, bra->ready, 0);
+    if (e == cudaSuccess && ket != bra) e = cudaStreamWaitEvent(st, ket->ready, 0);
+    if (e == cudaSuccess && bra->d.Ki * bra->d.Kj > 1 && ctx->tacc_used) e = cudaStreamWaitEvent(st, ctx->tacc_free, 0);
+    return e;
+}
+static cudaError_t order_after(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, cudaStream_t st) {
+    md4_pairs* b = const_cast<md4_pairs*>(bra);
+    md4_pairs* k = const_cast<md4_pairs*>(ket);
+    cudaError_t e = cudaSuccess;
+    if (bra->d.Ki * bra->d.Kj > 1) { e = cudaEventRecord(ctx->tacc_free, st); ctx->tacc_used = true; }
+    // a list read from several streams must outlive all of them: chain the new record behind the old one
+    if (e == cudaSuccess && b->used) e = cudaStreamWaitEvent(st, b->last_use, 0);
+    if (e == cudaSuccess) { e = cudaEventRecord(b->last_use, st); b->used = true; }
+    if (e == cudaSuccess && k != b) {
+        if (k->used) e = cudaStreamWaitEvent(st, k->last_use, 0);
+        if (e == cudaSuccess) { e = cudaEventRecord(k->last_use, st); k->used = true; }
+    }
+    return e;
+}
+
 md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out, size_t capacity_doubles,
                        void* cuda_stream) {
     size_t need = 0;
     md4_status s = check_compute(ctx, bra, ket, d_out, capacity_doubles, &need);
     if (s != MD4_OK || need == 0) return s;
     DeviceGuard g(ctx->device);
-    return launch_eri(ctx, bra->d, ket->d, d_out, (cudaStream_t)cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = order_before(ctx, bra, ket, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute", e);
+    s = launch_eri(ctx, bra->d, ket->d, d_out, st);
+    if (s != MD4_OK) return s;
+    e = order_after(ctx, bra, ket, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute", e);
+    return MD4_OK;
 }
 
 md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* h_out,
@@ -328,8 +484,10 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
     if (ctx->scratch_doubles < need) {
         cudaFree(ctx->d_scratch);
         ctx->d_scratch = nullptr; ctx->scratch_doubles = 0;
-        cudaError_t e = cudaMalloc((void**)&ctx->d_scratch, need * sizeof(double));
+        void* t = nullptr;
+        cudaError_t e = ctx_malloc(ctx, &t, need * sizeof(double));
         if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
+        ctx->d_scratch = static_cast<double*>(t);
         ctx->scratch_doubles = need;
     }
     // The bra list is cut into slices: the copy of slice i to the host (copy stream) runs under the kernel of
@@ -344,7 +502,7 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
     int nslice = 1;
     if (need * sizeof(double) >= ((size_t)64 << 20)) nslice = bra->d.npair < md4_ctx::NSLICE_EV ? bra->d.npair : md4_ctx::NSLICE_EV;
     const int kk = bra->d.Ki * bra->d.Kj;
-    cudaError_t e = cudaSuccess;
+    cudaError_t e = order_before(ctx, bra, ket, st);
     for (int i = 0; i < nslice && e == cudaSuccess; ++i) {
         const int b0 = (int)((long long)bra->d.npair * i / nslice), b1 = (int)((long long)bra->d.npair * (i + 1) / nslice);
         if (b1 == b0) continue;
@@ -364,6 +522,7 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
             e = cudaMemcpyAsync(h_out + (size_t)b0 * per_bra, d_slice, (size_t)(b1 - b0) * per_bra * sizeof(double),
                                 cudaMemcpyDeviceToHost, ctx->copy_stream);
     }
+    if (e == cudaSuccess) e = order_after(ctx, bra, ket, st);
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaError_t e3 = cudaStreamSynchronize(ctx->copy_stream);
     if (e == cudaSuccess) e = e2 != cudaSuccess ? e2 : e3;
@@ -431,6 +590,7 @@ md4_status md4_debug_pair_h(md4_ctx* ctx, const md4_pairs* pairs, int ipair, int
     const int kk = d.Ki * d.Kj;
     if (ipair < 0 || ipair >= d.npair || iprim < 0 || iprim >= kk) return fail(ctx, MD4_EINVAL, "md4_debug_pair_h: index out of range");
     DeviceGuard g(ctx->device);
+    if (pairs->ready) cudaEventSynchronize(pairs->ready);   // the pair kernel runs asynchronously on the build stream
     std::vector<double> blk(d.hstrideb), blk2(d.hstridek);
     double s8[8], pm = 0.0;
     const size_t ip = (size_t)ipair * kk + iprim;

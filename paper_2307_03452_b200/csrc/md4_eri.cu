@@ -21,9 +21,6 @@
 // Both contractions run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> SASS DMMA.8x8x4; tcgen05 has
 // no f64 kind on sm_100a, S: facts table).  (ab|cd) accumulates in registers over all primitive
 // quartets (Listing 2.1) and is written once.
-#ifdef MD4_PHASE_TIMING
-namespace md4 { __device__ unsigned long long g_phase[8]; }
-#endif
 #include "md4_device.cuh"
 
 namespace md4 {
@@ -80,15 +77,6 @@ __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterp
 
 // Position in the H_cd ring; every warp of the CTA (producer, consumers with and without rows) steps
 // through the same sequence of column blocks, so the positions stay equal without communication.
-#ifdef MD4_PHASE_TIMING
-// developer instrumentation (not compiled into the product): cycles per phase summed over consumer warps
-#define PT_DECL unsigned long long pt_t = clock64();
-#define PT_MARK(i) { const unsigned long long pt_n = clock64(); if (threadIdx.x % 32 == 0) atomicAdd(&g_phase[i], pt_n - pt_t); pt_t = pt_n; }
-#else
-#define PT_DECL
-#define PT_MARK(i)
-#endif
-
 struct RingPos {
     uint32_t s, ph;
     __device__ __forceinline__ void advance(uint32_t nst) {
@@ -119,7 +107,6 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
                                               bool load_t, bool last_kp) {
     double2 T[NQ];
     uint32_t aqr[NQ];
-    PT_DECL
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
         // [ab|q~] accumulates over the bra primitives (Listing 2.1 line 7): from the second one on the
@@ -163,7 +150,6 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
         for (int n = 0; n < NQ; ++n)
             if (!PRED || n < nq) dmma884(T[n].x, T[n].y, av.y, b[n]);
     }
-    PT_MARK(1)
     if (!last_kp) {
         // more bra primitives to come: park the partial [ab|q~]; the ket transform runs once per ket primitive
 #pragma unroll
@@ -178,9 +164,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
             const uint32_t m = lds_u32(c.sg32 + (uint32_t)(j0 + n) * 4u) >> (2 * c.k4);
             const double tx = (m & 1u) ? -T[n].x : T[n].x;
             const double ty = (m & 2u) ? -T[n].y : T[n].y;
-            PT_MARK(2)
             mbar_wait32(c.full32 + rp.s * 8u, rp.ph);
-            PT_MARK(3)
             const uint32_t bb = c.ring32 + rp.s * c.stage_bytes;
             constexpr int G = 4;   // B fragment pairs in flight
 #pragma unroll
@@ -201,7 +185,6 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
             rp.advance(c.nst);
         }
     }
-    PT_MARK(2)
 }
 
 template <int NT_CD, int NQT, int MAXW, bool EXACT, int MINB>
@@ -316,12 +299,9 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
 #pragma unroll
             for (int i = 0; i < NT_CD; ++i) acc[i] = make_double2(0.0, 0.0);
         }
-
-        PT_DECL
         __syncthreads();  // consumers are done with R of the previous primitive quartet, the builder with GA
         r_scatter(Ra, GA, sad, L, tid, nthr);
         __syncthreads();
-        PT_MARK(0)
 
         const bool last_kp = (kp == a.Kb - 1);   // the ket transform (and the ring) run with the last bra primitive only
         if (producer) {
@@ -426,8 +406,13 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
         return MD4_EUNSUPPORTED;
     }
     auto kern = eri_kernel<NT_CD, NQT, MAXW, EXACT, MINB>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lay.total);
-    if (e != cudaSuccess) { ctx->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return MD4_ECUDA; }
+    cudaError_t e = cudaSuccess;
+    // the shared-memory opt-in is a per-function attribute: set it once per context to the device maximum (never to a
+    // class-dependent value, which two contexts on one device could interleave), then launch with what the class needs
+    if (ctx->configured.insert(reinterpret_cast<const void*>(kern)).second) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin);
+        if (e != cudaSuccess) { ctx->configured.erase(reinterpret_cast<const void*>(kern)); ctx->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); return MD4_ECUDA; }
+    }
     const long long nwork = a.qmajor ? a.nquartets : a.nquartets * a.ncta_per_q;
     const long long slots = (long long)ctx->num_sms * MINB;
     long long grid = nwork < slots ? nwork : slots;
@@ -496,14 +481,6 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     return MD4_EUNSUPPORTED;
 }
 
-#ifdef MD4_PHASE_TIMING
-extern "C" void md4_debug_phase_cycles(unsigned long long* out8, int reset) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out8, g_phase, sizeof(g_phase));
-    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_phase, z, sizeof(z)); }
-}
-#endif
-
 // ---- stage-level debug kernels ---------------------------------------------------------------------
 namespace {
 __global__ void debug_boys_kernel(const double* tab, int mmax, int n, const double* T, double* out) {
@@ -545,7 +522,7 @@ cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, 
 
 cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out) {
     const size_t sm = ((size_t)r_alloc(L) + 2 * (size_t)n_hermite(L) + 32) * 8 + (size_t)n_hermite(L) * 6 + 16;
-    cudaError_t e = cudaFuncSetAttribute(debug_r_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    cudaError_t e = cudaFuncSetAttribute(debug_r_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin);
     if (e != cudaSuccess) return e;
     debug_r_kernel<<<1, 32, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, L, d_pq, d_out);
     ctx->launches++;

@@ -96,11 +96,24 @@ struct PairListDev {
     int* ij;             // [npair*2]
 };
 
+// One device allocation that the context may hand from a released pair list to the next one of (about) that size.
+// ev (may be null) completes when the last kernel that touches the block has finished; whoever reuses the block
+// makes its first writer wait for it (stream-ordered, the host never blocks).
+struct PoolBlock {
+    void* p = nullptr;
+    size_t bytes = 0;     // true size of the allocation
+    cudaEvent_t ev = nullptr;
+};
+
 }  // namespace md4
 
 struct md4_pairs {
     md4_ctx* ctx;
-    md4::PairListDev d;
+    md4::PairListDev d;          // views into `block`
+    md4::PoolBlock block;        // the list's single device allocation: Hb | Hk | scal | pairmax | ij
+    cudaEvent_t ready = nullptr;     // the pair kernel that fills the list has finished (recorded on ctx->build_stream)
+    cudaEvent_t last_use = nullptr;  // the last md4_compute that reads the list has finished (recorded on its stream)
+    bool used = false;
 };
 
 struct md4_ctx {
@@ -110,6 +123,13 @@ struct md4_ctx {
     std::vector<void*> table_allocs;
     // shells (device)
     int nshell = 0, nprim = 0;
+    // one device block (grows only) centres | exponents | coefficients | l | offsets, filled through a pinned staging
+    // buffer by a stream-ordered copy on build_stream, so replacing the shell set never synchronises the device
+    void* d_shell_block = nullptr;
+    size_t shell_block_bytes = 0;
+    void* h_shell_stage = nullptr;
+    size_t shell_stage_bytes = 0;
+    cudaEvent_t shell_done = nullptr;
     double* d_centers = nullptr;
     int* d_l = nullptr;
     int* d_off = nullptr;
@@ -117,11 +137,22 @@ struct md4_ctx {
     double* d_coef = nullptr;
     std::vector<int> h_l, h_off;
     std::set<md4_pairs*> lists;
-    // freed H buffers kept for the next md4_build_pairs (workspaces grow only, S:8(b)): a batch loop that
+    // released pair-list blocks kept for the next md4_build_pairs (workspaces grow only, S:8(b)): a batch loop that
     // builds and frees pair lists every step then never reaches cudaMalloc/cudaFree (both synchronise the device)
-    std::multimap<size_t, void*> pool;
-    size_t pool_bytes = 0;
+    std::multimap<size_t, md4::PoolBlock> pool;
+    size_t pool_bytes = 0, pool_max_bytes = 0;
+    cudaStream_t build_stream = nullptr;   // pair kernels run here; md4_compute waits for the lists' `ready` events
+    // pinned staging for the index lists of md4_build_pairs (the caller's array is copied during the call, the
+    // transfer to the device is stream-ordered): a slot is reused once its previous transfer has completed
+    static constexpr int NSTAGE = 4;
+    int* h_stage[NSTAGE] = {};
+    size_t stage_ints[NSTAGE] = {};
+    cudaEvent_t stage_done[NSTAGE] = {};
+    int stage_next = 0;
+    std::set<const void*> configured;      // kernels whose shared-memory opt-in has been set on this device
     double* d_tacc = nullptr;     // partial [ab|q~] of contracted bras, one slab per CTA of the fused kernel (md4_eri.cu)
+    cudaEvent_t tacc_free = nullptr;       // completes when the last launch that uses d_tacc has finished
+    bool tacc_used = false;
     double* d_scratch = nullptr;  // md4_compute_host staging
     size_t scratch_doubles = 0;
     static constexpr int NSLICE_EV = 8;   // md4_compute_host: bra slices whose D2H copy overlaps the next slice's kernel

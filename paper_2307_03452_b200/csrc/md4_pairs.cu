@@ -240,8 +240,10 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
     a.nab = pl.nab; a.nrb = pl.nrb; a.ncb = pl.ncbb; a.hstrideb = pl.hstrideb; a.hstridek = pl.hstridek;
     const size_t nblk = nprim * PAIR_SPLIT;
     if (nblk > 2147483647ull) return cudaErrorInvalidValue;
-    e = cudaFuncSetAttribute(pair_h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PairSmem));
-    if (e != cudaSuccess) return e;
+    if (ctx->configured.insert(reinterpret_cast<const void*>(pair_h_kernel)).second) {
+        e = cudaFuncSetAttribute(pair_h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PairSmem));
+        if (e != cudaSuccess) { ctx->configured.erase(reinterpret_cast<const void*>(pair_h_kernel)); return e; }
+    }
     pair_h_kernel<<<(unsigned)nblk, PAIR_THREADS, sizeof(PairSmem), st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();

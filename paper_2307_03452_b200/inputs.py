@@ -128,12 +128,12 @@ def sweep_classes():
     return [(a, b, c, d) for (a, b) in prs for (c, d) in prs if (a, b) >= (c, d)]
 
 
-def config5(class_index: int, K: int = 1, nper: int = 8) -> Workload:
+def config5(class_index: int, K: int = 1, nper: int = 8, seed_offset: int = 0) -> Workload:
     """One class of the mixed sweep: nper shells per role a,b,c,d (box 10), bra = all nper x nper (a_i,b_j),
     ket = all (c_i,d_j); K = 1: exponents in [0.05, 50]; K = 3: zeta_0 in [0.05, 50/9], ratio 3;
     seed 1000 + class index."""
     la, lb, lc, ld = sweep_classes()[class_index]
-    seed = 1000 + class_index
+    seed = 1000 + class_index + seed_offset   # seed_offset: other ranks of a multi-GPU bench draw their own shells
     rng = np.random.Generator(np.random.PCG64(seed))
     ls = np.repeat(np.array([la, lb, lc, ld], dtype=np.int32), nper)
     hi = 50.0 if K == 1 else 50.0 / 9.0

@@ -20,6 +20,7 @@ STATUS_NAMES = ["MD4_OK", "MD4_EINVAL", "MD4_EUNSUPPORTED", "MD4_ESTATE", "MD4_E
 #: every symbol include/md4.h declares (tests check the library exports exactly these)
 SYMBOLS = [
     "md4_create", "md4_destroy", "md4_last_error", "md4_set_shells", "md4_build_pairs", "md4_free_pairs",
+    "md4_stream_wait_pairs",
     "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host",
     "md4_launch_count", "md4_flops_per_quartet", "md4_debug_boys", "md4_debug_solid_coeff",
     "md4_debug_hermite_r", "md4_debug_pair_h", "md4_debug_work_items",
@@ -56,6 +57,8 @@ def load():
     lib.md4_build_pairs.restype = ctypes.c_int
     lib.md4_free_pairs.argtypes = [vp, vp]
     lib.md4_free_pairs.restype = None
+    lib.md4_stream_wait_pairs.argtypes = [vp, vp, vp]
+    lib.md4_stream_wait_pairs.restype = ctypes.c_int
     lib.md4_pairs_count.argtypes = [vp]
     lib.md4_pairs_count.restype = ctypes.c_int
     lib.md4_pairs_class.argtypes = [vp, ip]
@@ -169,6 +172,9 @@ class Engine:
         h = ctypes.c_void_p()
         self._check(load().md4_build_pairs(self.handle, int(a.shape[0]), _ip(a), ctypes.byref(h)))
         return PairList(self, h)
+
+    def stream_wait_pairs(self, pairs: PairList, stream: int):
+        self._check(load().md4_stream_wait_pairs(self.handle, pairs.handle, ctypes.c_void_p(stream)))
 
     def output_size(self, bra: PairList, ket: PairList) -> int:
         n = ctypes.c_size_t()

@@ -54,6 +54,8 @@ def time_workload(eng, wl, reps: int):
     p0.record(stream)
     bra = eng.build_pairs(wl.bra_ij)
     ket = eng.build_pairs(wl.ket_ij)
+    eng.stream_wait_pairs(bra, stream.cuda_stream)   # the pair kernels run on the engine's own stream
+    eng.stream_wait_pairs(ket, stream.cuda_stream)
     p1.record(stream)
     torch.cuda.synchronize()
     pair_ms = p0.elapsed_time(p1)

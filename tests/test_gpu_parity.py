@@ -187,29 +187,59 @@ def test_config2_sampled(eng):
 
 
 def test_config3_sampled(eng):
-    """cfg 3 (ii|ii) K=1, the headline workload, full 16384-quartet launch; 96 sampled quartets + corners."""
+    """cfg 3 (ii|ii) K=1, the headline workload, full 16384-quartet launch (the launch bench.py times); 384 sampled
+    quartets + corners, among them quartets of every CTA's first and later passes through the persistent grid."""
     wl = inputs.config3()
-    errs, below = _sampled(eng, wl, 96, 103, extra=(0, 127, 128, wl.nquartets - 1))
+    errs, below = _sampled(eng, wl, 384, 103, extra=(0, 73, 74, 127, 128, 147, 148, wl.nquartets - 1))
     assert errs.max() <= TOL, errs.max()
 
 
 def test_config4_sampled(eng):
-    """cfg 4 (ii|ii) K=5 per shell (625 primitive quartets): 1024-quartet launch, 2 quartets vs the oracle
-    (binary128: ~6 CPU-minutes per quartet, primitive loop spread over 16 threads)."""
+    """cfg 4 (ii|ii) K=5 per shell (625 primitive quartets, Listing 2.1): the full 1024-quartet launch bench.py
+    would time, 8 quartets vs the binary128 oracle (~6 CPU-minutes each, primitive loop spread over the host threads).
+    The persistent grid has 148 CTAs and a quartet is two work items, so quartets >= 74 are computed by a CTA that has
+    already finished another item and re-uses its [ab|q~] scratch slab: 6 of the 8 sampled quartets are of that kind
+    (first item after the wrap, second wrap, middle, last)."""
     wl = inputs.config4()
-    errs, below = _sampled(eng, wl, 1, 104, extra=(0,), nslice=16)
-    assert errs.max() <= TOL, errs.max()
-
-
-@pytest.mark.parametrize("ci", [1, 7, 12, 19])
-def test_config5_classes_k3(eng, ci):
-    """cfg 5 mixed classes at K = 3 per shell (81 primitive quartets), reduced to 3 x 3 pairs for oracle time."""
-    wl = inputs.config5(ci, K=3)
-    wl.bra_ij = wl.bra_ij[[0, 9, 63]]
-    wl.ket_ij = wl.ket_ij[[5, 18, 60]]
-    g, r = _run(eng, wl, nslice=4)
+    sub = [0, 73, 74, 147, 148, 500, 777, wl.nquartets - 1]
+    g, r = _run(eng, wl, subset=sub, nslice=16)
     errs, below = _quartet_errors(g, r)
-    assert errs.max() <= TOL, (wl.name, errs.max())
+    assert errs.max() <= TOL, errs
+
+
+def test_config4_full_launch_equals_per_bra_launches(eng):
+    """Self-consistency of the persistent grid at K > 1 on ALL 1024 quartets of cfg 4: in one launch a CTA walks
+    through ~14 work items, parking and reloading partial [ab|q~] sums in its scratch slab; in 32 launches of one bra
+    pair each (64 items < 148 CTAs) no CTA ever takes a second item.  The summation order per quartet is the same, so
+    the two results must be bit-identical; a stale or wrong slab on a later item would show here."""
+    import torch
+
+    wl = inputs.config4()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    full = eng.compute(bra, ket)
+    torch.cuda.synchronize()
+    for i in range(len(wl.bra_ij)):
+        b1 = eng.build_pairs(wl.bra_ij[i:i + 1])
+        one = eng.compute(b1, ket)
+        torch.cuda.synchronize()
+        assert torch.equal(one[0], full[i]), f"bra pair {i}: full launch differs from the single-bra launch"
+        b1.free()
+    bra.free(); ket.free()
+
+
+@pytest.mark.parametrize("ci", list(range(21)))
+def test_config5_classes_k3(eng, ci):
+    """cfg 5, all 21 classes at K = 3 per shell (81 primitive quartets): the full 64 x 64 launch, 4 quartets vs the
+    binary128 oracle: the first, the last, and two with index >= 148, i.e. computed in a CTA's second or later pass
+    through the 148-CTA persistent grid whichever way the class splits a quartet into work items."""
+    wl = inputs.config5(ci, K=3)
+    rng = np.random.Generator(np.random.PCG64(700 + ci))
+    sub = np.unique(np.concatenate([[0, wl.nquartets - 1], rng.choice(np.arange(148, wl.nquartets - 1), size=2, replace=False)]))
+    g, r = _run(eng, wl, subset=sub, nslice=4)
+    errs, below = _quartet_errors(g, r)
+    assert errs.max() <= TOL, (wl.name, errs)
 
 
 @pytest.mark.parametrize("ci", list(range(21)))
@@ -329,3 +359,63 @@ def test_compute_host_sliced_matches_device(eng):
     assert eng.launch_count() - n0 == 8
     assert np.array_equal(d.cpu().numpy(), h)
     bra.free(); ket.free()
+
+
+def test_two_streams_contracted_bras_do_not_race(eng):
+    """Two md4_compute calls with contracted bras (K_bra > 1: the partial [ab|q~] sums go through the context's scratch
+    buffer) enqueued back to back on two different streams of one context: both results must match the oracle, and the
+    repeat on one stream bit for bit.  Without the internal ordering the second launch would overwrite the first one's
+    scratch slabs while it runs."""
+    import torch
+
+    wlA = inputs.small_workload((6, 6, 6, 6), (2, 2, 1, 1), nbra=20, nket=20, seed=31)
+    wlB = inputs.small_workload((6, 5, 5, 4), (3, 1, 1, 2), nbra=20, nket=20, seed=32)
+    res = {}
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    lists = []
+    for tag, wl, st in (("A", wlA, s1), ("B", wlB, s2)):
+        s = wl.shells
+        eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+        bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+        lists += [bra, ket]
+        res[tag] = [eng.compute(bra, ket, stream=st.cuda_stream)]
+        # a second launch of the same batch on the OTHER stream, while the first may still be running
+        other = s2 if st is s1 else s1
+        res[tag].append(eng.compute(bra, ket, stream=other.cuda_stream))
+    torch.cuda.synchronize()
+    for tag, wl in (("A", wlA), ("B", wlB)):
+        assert torch.equal(res[tag][0], res[tag][1]), tag
+        g = res[tag][0].cpu().numpy()
+        sub = np.array([0, 147, 148, 399], dtype=np.int32)
+        ref = oracle.compute(_oshells(wl.shells), wl.bra_ij, wl.ket_ij, subset=sub, nslice=2)
+        errs, _ = _quartet_errors(g.reshape((400,) + g.shape[2:])[sub], ref)
+        assert errs.max() <= TOL, (tag, errs)
+    for pl in lists:
+        pl.free()
+
+
+def test_free_and_rebuild_without_host_sync(eng):
+    """md4_free_pairs hands a list's memory to the next md4_build_pairs while the compute that reads it may still be
+    running (device-side event ordering, no host synchronisation): results of a build/compute/free loop that is never
+    synchronised in between must equal the synchronised ones."""
+    import torch
+
+    wl = inputs.config2()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    ref = eng.compute(bra, ket).clone()
+    torch.cuda.synchronize()
+    bra.free(); ket.free()
+    outs = []
+    for it in range(4):
+        # alternate the roles so that a recycled block is overwritten with DIFFERENT data while its old reader runs
+        b_ij, k_ij = (wl.bra_ij, wl.ket_ij) if it % 2 == 0 else (wl.ket_ij, wl.bra_ij)
+        bra, ket = eng.build_pairs(b_ij), eng.build_pairs(k_ij)
+        outs.append(eng.compute(bra, ket))
+        bra.free(); ket.free()
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0], ref) and torch.equal(outs[2], ref)
+    assert torch.equal(outs[1], outs[3])
+    assert torch.equal(outs[1].permute(1, 0, 4, 5, 2, 3).contiguous(), ref) or \
+        (outs[1].permute(1, 0, 4, 5, 2, 3) - ref).abs().max() <= 1e-12 * ref.abs().max()

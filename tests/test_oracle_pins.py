@@ -350,3 +350,38 @@ def test_batch_driver_slices_and_precisions():
         assert np.array_equal(full[0, 0], one)
         sub = oracle.compute(sh2, b, ket, subset=[0], nthreads=1)
         assert np.array_equal(sub[0], full[0, 0])
+
+
+def test_batch_driver_addressing_on_ragged_lists():
+    """oracle.compute writes out[i_bra][j_ket] (the md4_compute layout, include/md4.h): a 2 x 3 list with distinct
+    shells on every pair, each slot against its own oracle.quartet call (the per-quartet routine is what the other
+    pins check); an i/j transposition or a wrong stride in the batch driver would fail here.  Also the subset form
+    out[k] = quartet subset[k] in the caller's order, and sliced primitive loops on the same lists."""
+    rng = np.random.default_rng(78)
+    n = 6
+    cent = rng.uniform(0, 2.5, (n, 3))
+    ls = np.array([2, 2, 2, 1, 1, 1], dtype=np.int32)           # bra pairs (d,p), ket pairs (p,d)
+    K = [1, 2, 1, 2, 1, 1]                                      # shells 1 and 3 (unused) shift the primitive offsets
+    off = np.concatenate([[0], np.cumsum(K)]).astype(np.int32)
+    ex = np.exp(rng.uniform(math.log(0.3), math.log(3.0), off[-1]))
+    co = rng.uniform(0.3, 1.0, off[-1])
+    sh = oracle.Shells(cent, ls, off, ex, co)
+    bra = np.array([[0, 4], [2, 5]], dtype=np.int32)           # both (l=2,K=1 | l=1,K=1)
+    ket = np.array([[4, 0], [5, 2], [4, 2]], dtype=np.int32)   # all (l=1,K=1 | l=2,K=1), three different pairs
+    full = oracle.compute(sh, bra, ket, nthreads=3)
+    assert full.shape == (2, 3, 5, 3, 3, 5)
+    for i, (a, b) in enumerate(bra):
+        for j, (c, d) in enumerate(ket):
+            one = oracle.quartet(sh, int(a), int(b), int(c), int(d), quad=True).astype(np.float64)
+            assert np.array_equal(full[i, j], one), (i, j)
+    # the six quartets are pairwise different, so a transposed or shifted slot cannot pass by accident
+    flat = full.reshape(6, -1)
+    for x in range(6):
+        for y in range(x + 1, 6):
+            assert np.abs(flat[x] - flat[y]).max() > 1e-6 * np.abs(flat[x]).max()
+    order = [5, 0, 3]
+    sub = oracle.compute(sh, bra, ket, subset=order, nthreads=2)
+    for k, f in enumerate(order):
+        assert np.array_equal(sub[k], full[f // 3, f % 3])
+    sliced = oracle.compute(sh, bra, ket, subset=order, nthreads=4, nslice=3)
+    assert np.abs(sliced - sub).max() <= 1e-16 * np.abs(sub).max()
