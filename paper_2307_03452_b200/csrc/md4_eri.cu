@@ -44,6 +44,7 @@ struct EriArgs {
     int row0[3], nrows[3];   // 8-row blocks of ab of the ncta_per_q work items of one quartet (plan_items)
     long long nquartets;
     int qmajor;   // 1: a CTA takes whole quartets (items of unequal size); 0: the items of a quartet go to neighbouring CTAs
+    int tb;       // bra pairs per strip of the quartet order (quartet_pairs)
     const uint32_t* rtab; const uint32_t* tuv; const double* boys;
     double* tacc;   // [grid][wpc][ncb_q][32][2] partial [ab|q~] of contracted bras
     const uint32_t* colp; const uint32_t* colq;   // bra-order columns of the bra class, ket-order columns of the ket class
@@ -74,6 +75,21 @@ struct SmemLayout {
 };
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+
+// Order in which the persistent grid walks the quartets: the bra list is cut into strips of tb pairs and a strip is walked
+// ket-major, so the ~74 quartets the 148 CTAs work on at any time are tb bra pairs x 2-3 ket pairs: their H matrices
+// (0.6 MB each for ii) stay in L2 while they are in use, every H_cd is read from HBM once per strip and every H_ab once.
+// (Walking the flat list [bra][ket] put one bra and 74 different kets in flight and re-read H_cd from HBM 28 times over:
+// 8.6 GB per cfg3 launch against 0.3 GB of pair data, profiles/r1_eri_kernel_ncu.md.)
+__device__ __forceinline__ void quartet_pairs(const EriArgs& a, long long q, int& ib, int& jk) {
+    const long long per_strip = (long long)a.tb * a.nket;
+    const int strip = (int)(q / per_strip);
+    const int r = (int)(q - strip * per_strip);
+    const int b0 = strip * a.tb;
+    const int hb = min(a.tb, a.nbra - b0);
+    jk = r / hb;
+    ib = b0 + r % hb;
+}
 
 // Position in the H_cd ring; every warp of the CTA (producer, consumers with and without rows) steps
 // through the same sequence of column blocks, so the positions stay equal without communication.
@@ -181,7 +197,11 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
                     if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) dmma884(acc[nb0 + g].x, acc[nb0 + g].y, ty, bv[g].y);
             }
             __syncwarp();
-            if (c.lane == 0) mbar_arrive32(c.empty32 + rp.s * 8u);
+            // release the stage.  The arrive takes the last accumulator of the q-block as a (fake) input: it cannot be
+            // scheduled before the last DMMA, i.e. before every B fragment of the stage has been read into registers.
+            // (Without it ptxas places the arrive right behind the ISSUE of the last LDS, ahead of the DMMAs that wait for
+            // the data: the producer may then refill the stage while loads of it are still in flight.)
+            if (c.lane == 0) mbar_arrive32_after(c.empty32 + rp.s * 8u, acc[NT_CD - 1].x, acc[NT_CD - 1].y);
             rp.advance(c.nst);
         }
     }
@@ -255,8 +275,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
 
     // builds R of primitive quartet (it, q, p) into GA; poll() is called between batches
     auto build_r = [&](long long it, int q, int p, auto poll) {
-        const long long qt = it;
-        const int ib = (int)(qt / a.nket), jk = (int)(qt % a.nket);
+        int ib, jk;
+        quartet_pairs(a, it, ib, jk);
         const double* sp = a.sb + ((size_t)ib * a.Kb + p) * 8;
         const double* sq = a.sk + ((size_t)jk * a.Kk + q) * 8;
         hermite_r_warp(GA, sS, srt, a.boys, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
@@ -292,7 +312,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
         const bool nhave = nquartet < a.nquartets;
         const bool item_ends = (nquartet != quartet) || (nms != ms);
 
-        const int ib = (int)(quartet / a.nket), jk = (int)(quartet % a.nket);
+        int ib, jk;
+        quartet_pairs(a, quartet, ib, jk);
         const int mbk = (ms == 0 ? a.row0[0] : (ms == 1 ? a.row0[1] : a.row0[2])) + warp;   // 8-row block of ab owned by this warp
         const bool active = !producer && warp < (ms == 0 ? a.nrows[0] : (ms == 1 ? a.nrows[1] : a.nrows[2]));
         if (kq == 0 && kp == 0) {
@@ -353,13 +374,31 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
             if (item_ends) {
                 const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
                 const int row = mbk * 8 + (lane >> 2);
-                if (row < a.nab) {
-                    double* o = a.out + (size_t)quartet * a.nab * a.ncd + (size_t)row * a.ncd;
+                // (a9) 16-byte streaming stores (st.global.cs.v2.f64: the 3.7 GB output stream must not evict H from L2).
+                // A lane holds columns (c, c+1), c = 8 nb + 2 k4, of its row; rows start at element (quartet Nab + row) Ncd of
+                // the output, which is odd for every other row when Ncd is odd: there the aligned pairs are (c+1, c+2), whose
+                // second element comes from the neighbouring lane (or, for k4 = 3, from this row's first lane, next block).
+                const size_t e0 = ((size_t)ib * a.nket + jk) * a.nab * a.ncd + (size_t)(row < a.nab ? row : 0) * a.ncd;
+                double* o = a.out + e0;
+                const bool odd = ((reinterpret_cast<uintptr_t>(o) >> 3) & 1) != 0;   // d_out itself need only be 8-byte aligned
+                const bool rowok = row < a.nab;
 #pragma unroll
-                    for (int nb = 0; nb < NT_CD; ++nb) {
-                        const int col = nb * 8 + 2 * cc.k4;
-                        if (col < a.ncd) __stcs(o + col, (acc[nb].x * f) * f);   // streaming store: the output must not evict H from L2
-                        if (col + 1 < a.ncd) __stcs(o + col + 1, (acc[nb].y * f) * f);
+                for (int nb = 0; nb < NT_CD; ++nb) {
+                    const double vx = (acc[nb].x * f) * f, vy = (acc[nb].y * f) * f;
+                    const double nx_same = __shfl_sync(0xffffffffu, vx, (lane & ~3) | ((cc.k4 + 1) & 3));
+                    double nx_next = 0.0;
+                    if (nb + 1 < NT_CD) nx_next = __shfl_sync(0xffffffffu, (acc[nb + 1].x * f) * f, lane & ~3);
+                    const double nx = cc.k4 == 3 ? nx_next : nx_same;
+                    const int col = nb * 8 + 2 * cc.k4;
+                    if (rowok) {
+                        if (!odd) {
+                            if (col + 1 < a.ncd) __stcs(reinterpret_cast<double2*>(o + col), make_double2(vx, vy));
+                            else if (col < a.ncd) __stcs(o + col, vx);
+                        } else {
+                            if (col == 0) __stcs(o, vx);
+                            if (col + 2 < a.ncd) __stcs(reinterpret_cast<double2*>(o + col + 1), make_double2(vy, nx));
+                            else if (col + 1 < a.ncd) __stcs(o + col + 1, vy);
+                        }
                     }
                 }
             }
@@ -459,6 +498,7 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     plan_items(a);
     a.nquartets = (long long)a.nbra * a.nket;
     a.qmajor = (a.ncta_per_q == 2 && a.nrows[0] != a.nrows[1]) ? 1 : 0;
+    a.tb = 32;
     a.nst = 2;
     a.rtab = ctx->tab.rtab; a.tuv = ctx->tab.tuv; a.boys = ctx->tab.boys;
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];

@@ -419,3 +419,26 @@ def test_free_and_rebuild_without_host_sync(eng):
     assert torch.equal(outs[1], outs[3])
     assert torch.equal(outs[1].permute(1, 0, 4, 5, 2, 3).contiguous(), ref) or \
         (outs[1].permute(1, 0, 4, 5, 2, 3) - ref).abs().max() <= 1e-12 * ref.abs().max()
+
+
+@pytest.mark.parametrize("which", ["cfg4", "cfg5 (ii|hh) K=3", "cfg5 (ii|ii) K=3", "cfg3"])
+def test_repeated_launches_are_bit_identical(eng, which):
+    """Every quartet is computed by one CTA in a fixed summation order, so two launches of the same batch must agree bit
+    for bit on EVERY element.  This is the test that exposed a write-after-read race on the H_cd ring in round 2 (the
+    assembler had moved the release of a ring stage ahead of the tensor instructions that wait for the stage's last
+    loads; contracted classes with spilled accumulators then read refilled data now and then: errors of 1e-9 ... O(1) in
+    a few dozen of 1024 quartets, which the sampled oracle comparisons never hit).  Full launches, all elements."""
+    import torch
+
+    wl = {"cfg4": inputs.config4, "cfg3": inputs.config3, "cfg5 (ii|hh) K=3": lambda: inputs.config5(17, K=3),
+          "cfg5 (ii|ii) K=3": lambda: inputs.config5(20, K=3)}[which]()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    ref = eng.compute(bra, ket).clone()
+    torch.cuda.synchronize()
+    for rep in range(3):
+        out = eng.compute(bra, ket)
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref), f"{which}: launch {rep + 2} differs from the first in {int((out != ref).sum())} elements"
+    bra.free(); ket.free()
