@@ -61,6 +61,10 @@ def _bind(lib):
         i_p = ctypes.POINTER(ctypes.c_int)
         lib.oracle_boys.argtypes = [ctypes.c_int, ctypes.c_longdouble, ld_p]
         lib.oracle_boys.restype = None
+        lib.oracle_set_kernel.argtypes = [ctypes.c_int, ctypes.c_double]
+        lib.oracle_set_kernel.restype = ctypes.c_int
+        lib.oracle_kernel_seeds.argtypes = [ctypes.c_int, ctypes.c_longdouble, ctypes.c_longdouble, ld_p]
+        lib.oracle_kernel_seeds.restype = None
         lib.oracle_solid_coeff.argtypes = [ctypes.c_int, ld_p]
         lib.oracle_solid_coeff.restype = None
         lib.oracle_cart_pos.argtypes = [ctypes.c_int] * 3
@@ -90,6 +94,25 @@ def boys(mmax: int, T) -> np.ndarray:
     (ctypes converts through Python float), evaluated in long double."""
     out = np.zeros(mmax + 1, dtype=np.longdouble)
     _load().oracle_boys(int(mmax), ctypes.c_longdouble(float(T)), _ld(out))
+    return out
+
+
+KERNELS = {"coulomb": 0, "erf": 1, "erfc": 2}
+
+
+def set_kernel(kind: str = "coulomb", omega: float = 0.0) -> None:
+    """Interaction kernel of every later call, in BOTH builds: 1/r ("coulomb"), erf(omega r)/r or erfc(omega r)/r
+    (ref. 21: only the seeds [0]^(m) change, see eri_oracle.c)."""
+    for quad in (False, True):
+        rc = _load(quad).oracle_set_kernel(KERNELS[kind], float(omega))
+        if rc:
+            raise ValueError(f"bad kernel {kind!r}, omega = {omega}")
+
+
+def kernel_seeds(mmax: int, rho: float, T: float) -> np.ndarray:
+    """G_m(rho, T), m = 0..mmax, for the current kernel (long-double build)."""
+    out = np.zeros(mmax + 1, dtype=np.longdouble)
+    _load().oracle_kernel_seeds(int(mmax), ctypes.c_longdouble(float(rho)), ctypes.c_longdouble(float(T)), _ld(out))
     return out
 
 

@@ -136,6 +136,52 @@ static void boys_real(int mmax, real T, real *F)
     for (int m = mmax - 1; m >= 0; --m) F[m] = (2.0L * T * F[m + 1] + eT) / (2 * m + 1);
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * Interaction kernel g(r12) ("[0]^(m) is related to the Boys function (or similar quantities for
+ * non-Coulomb integrals, ref. 21)").  Ref. 21 (Ahlrichs 2006) shows that for g(r) = Int w(u) exp(-u^2 r^2) du the
+ * Obara-Saika recurrences are unchanged and only the seeds change: with y^2 = u^2/(rho + u^2),
+ *     [00|00]^(m) = prefactor * G_m,   G_m = Int_0^1 w~(y) y^{2m} exp(-T y^2) dy.
+ *   Coulomb 1/r:            w~ = 1 on [0,1]          G_m = F_m(T)
+ *   erf(omega r)/r:         w~ = 1 on [0,s], else 0   G_m = s^{2m+1} F_m(s^2 T),  s^2 = omega^2/(omega^2 + rho)
+ *   erfc(omega r)/r:        the difference            G_m = F_m(T) - s^{2m+1} F_m(s^2 T)
+ * (substitute y = s y' in the truncated integral).  Process-wide setting, read when a quartet starts.
+ * Pinned in tests/test_oracle_pins.py: G_m against mpmath quadrature of the truncated integral, (ab|cd) against the
+ * brute-force quadrature of tests/refquad.py with the u-integral cut at omega, erf + erfc = Coulomb, omega -> infinity.
+ * ---------------------------------------------------------------------------------------------- */
+static int g_kernel_kind = 0;          /* 0 Coulomb, 1 erf-attenuated, 2 erfc-attenuated */
+static double g_kernel_omega = 0.0;
+int oracle_set_kernel(int kind, double omega)
+{
+    if (kind < 0 || kind > 2 || (kind != 0 && !(omega > 0.0))) return 1;
+    g_kernel_kind = kind; g_kernel_omega = omega;
+    return 0;
+}
+
+/* G_m, m = 0..mmax, for the current kernel */
+static void kernel_seeds(int mmax, real rho, real T, real *G)
+{
+    boys_real(mmax, T, G);
+    if (g_kernel_kind == 0) return;
+    real w2 = (real)g_kernel_omega * (real)g_kernel_omega;
+    real s2 = w2 / (w2 + rho), sp = R_SQRT(s2);      /* sp = s^{2m+1} */
+    real *H = (real *)malloc(sizeof(real) * (mmax + 1));
+    boys_real(mmax, s2 * T, H);
+    for (int m = 0; m <= mmax; ++m) {
+        real att = sp * H[m];
+        G[m] = g_kernel_kind == 1 ? att : G[m] - att;
+        sp *= s2;
+    }
+    free(H);
+}
+
+void oracle_kernel_seeds(int mmax, long double rho, long double T, long double *G)
+{
+    real *tmp = (real *)malloc(sizeof(real) * (mmax + 1));
+    kernel_seeds(mmax, (real)rho, (real)T, tmp);
+    for (int m = 0; m <= mmax; ++m) G[m] = (long double)tmp[m];
+    free(tmp);
+}
+
 void oracle_boys(int mmax, long double T, long double *F)
 {
     real *tmp = (real *)malloc(sizeof(real) * (mmax + 1));
@@ -257,7 +303,7 @@ static int quartet_cart_dir(const shell_t *sa, const shell_t *sb, const shell_t 
         /* step 2 */
         real pref = (real)sa->coefs[ka] * sb->coefs[kb] * sc->coefs[kc] * sd->coefs[kd] * Kab * Kcd *
                     2.0L * R_POW(pi, 2.5L) / (p * q * R_SQRT(p + q));
-        boys_real(L, T, F);
+        kernel_seeds(L, rho, T, F);     /* F_m(T) for the Coulomb kernel */
         for (int m = 0; m <= L; ++m) VV(0, 0, m) = pref * F[m];
         /* step 3a: [e+1_i,0|00]^(m) = PA_i [e0|00]^(m) + WP_i [e0|00]^(m+1)
          *                            + e_i/(2p) ( [e-1_i,0|00]^(m) - rho/p [e-1_i,0|00]^(m+1) )           */

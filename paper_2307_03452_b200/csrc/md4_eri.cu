@@ -498,7 +498,14 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     plan_items(a);
     a.nquartets = (long long)a.nbra * a.nket;
     a.qmajor = (a.ncta_per_q == 2 && a.nrows[0] != a.nrows[1]) ? 1 : 0;
-    a.tb = 32;
+    // strip height: the H matrices of a strip's bra pairs (K_bra matrices each) should stay L2-resident next to the kets
+    // in flight: <= 16 MB per strip.  Measured on cfg3 / cfg5 (ii|ii) K=3: flat order 58.0 / 923 ms, 32-pair strips
+    // 57.8 / 962 ms (a contracted strip of 32 is 185 MB), this rule 57.8 / 923 ms.
+    {
+        const double bytes_per_bra = (double)a.Kb * (double)a.hsb * sizeof(double);
+        int tb = (int)(16.0 * 1024 * 1024 / bytes_per_bra);
+        a.tb = tb < 1 ? 1 : (tb > 32 ? 32 : tb);
+    }
     a.nst = 2;
     a.rtab = ctx->tab.rtab; a.tuv = ctx->tab.tuv; a.boys = ctx->tab.boys;
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];

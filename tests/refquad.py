@@ -51,9 +51,11 @@ def _axis_integrals(la, lb, lc, ld, za, zb, zc, zd, A, B, C, D, u2, ngh):
     return out
 
 
-def eri_cart_quadrature(ls, zs, centers, cart_lists, ngl=120, ngh=None):
+def eri_cart_quadrature(ls, zs, centers, cart_lists, ngl=120, ngh=None, kernel="coulomb", omega=None):
     """Unnormalised primitive Cartesian block [a b|c d]: array [na, nb, nc, nd] in the order of ``cart_lists``
-    (four lists of (x,y,z) exponent triples)."""
+    (four lists of (x,y,z) exponent triples).  kernel: "coulomb" 1/r12; "erf": erf(omega r12)/r12 = (2/sqrt(pi))
+    Int_0^omega exp(-u^2 r12^2) du, i.e. the same u-integral cut at u = omega (t <= omega/sqrt(rho + omega^2));
+    "erfc": the rest of the u-range."""
     la, lb, lc, ld = ls
     za, zb, zc, zd = zs
     A, B, C, D = [np.asarray(c, dtype=float) for c in centers]
@@ -62,8 +64,12 @@ def eri_cart_quadrature(ls, zs, centers, cart_lists, ngl=120, ngh=None):
     p, q = za + zb, zc + zd
     rho = p * q / (p + q)
     t, wt = np.polynomial.legendre.leggauss(ngl)
-    t = 0.5 * (t + 1.0)
-    wt = 0.5 * wt
+    t0, t1 = 0.0, 1.0
+    if kernel != "coulomb":
+        tc = omega / math.sqrt(rho + omega * omega)
+        t0, t1 = (0.0, tc) if kernel == "erf" else (tc, 1.0)
+    t = t0 + (t1 - t0) * 0.5 * (t + 1.0)
+    wt = (t1 - t0) * 0.5 * wt
     u2 = rho * t * t / (1.0 - t * t)
     dudt = math.sqrt(rho) * (1.0 - t * t) ** -1.5
     I = [_axis_integrals(la, lb, lc, ld, za, zb, zc, zd, A[i], B[i], C[i], D[i], u2, ngh) for i in range(3)]

@@ -385,3 +385,68 @@ def test_batch_driver_addressing_on_ragged_lists():
         assert np.array_equal(sub[k], full[f // 3, f % 3])
     sliced = oracle.compute(sh, bra, ket, subset=order, nthreads=4, nslice=3)
     assert np.abs(sliced - sub).max() <= 1e-16 * np.abs(sub).max()
+
+
+# ------------------------------------------------ non-Coulomb kernels (ref. 21)
+@pytest.fixture
+def coulomb_after():
+    yield
+    oracle.set_kernel("coulomb")
+
+
+def test_kernel_seeds_vs_truncated_boys_integral(coulomb_after):
+    """G_m = Int_0^s y^2m exp(-T y^2) dy (erf), Int_s^1 (erfc), s^2 = omega^2/(omega^2 + rho): mpmath quadrature of the
+    defining integral at 30 digits (library routine) against the oracle's s^(2m+1) F_m(s^2 T) form."""
+    import mpmath as mp
+
+    mp.mp.dps = 30
+    for omega, rho, T in [(0.3, 0.7, 0.0), (0.3, 0.7, 2.5), (1.1, 0.05, 40.0), (0.2, 25.0, 130.0), (5.0, 1.0, 9.0)]:
+        s = mp.sqrt(mp.mpf(omega) ** 2 / (mp.mpf(omega) ** 2 + mp.mpf(rho)))
+        for kind, (lo, hi) in (("erf", (0, s)), ("erfc", (s, 1))):
+            oracle.set_kernel(kind, omega)
+            G = oracle.kernel_seeds(12, rho, T)
+            for m in (0, 1, 5, 12):
+                ref = mp.quad(lambda y: y ** (2 * m) * mp.exp(-mp.mpf(T) * y * y), [lo, hi])
+                got = mp.mpf(np.format_float_scientific(G[m], precision=25, unique=False))
+                # a few long-double ulps of the value, plus (erfc is a difference) of the full Boys integral it is cut from
+                full = mp.quad(lambda y: y ** (2 * m) * mp.exp(-mp.mpf(T) * y * y), [0, 1])
+                assert abs(got - ref) <= mp.mpf("1e-17") * abs(ref) + mp.mpf("5e-19") * full, (kind, omega, rho, T, m)
+
+
+@pytest.mark.parametrize("kind", ["erf", "erfc"])
+@pytest.mark.parametrize("ls", [(0, 0, 0, 0), (1, 1, 1, 1), (2, 1, 0, 2)])
+def test_attenuated_kernels_vs_bruteforce_quadrature(coulomb_after, kind, ls):
+    """(ab|cd) with erf(omega r12)/r12 and erfc(omega r12)/r12 against the brute-force quadrature of refquad.py with the
+    u-integral of 1/r12 = (2/sqrt pi) Int exp(-u^2 r12^2) du cut at omega: uses neither Boys nor any recurrence."""
+    rng = np.random.default_rng(91)
+    sh = _rand_shells(rng, list(ls))
+    omega = 0.6
+    oracle.set_kernel(kind, omega)
+    got = oracle.quartet(sh, 0, 1, 2, 3, solid=False).astype(np.float64) / np.prod(sh.coefficients)
+    cls = [oracle.cart_list(l) for l in ls]
+    ref = refquad.eri_cart_quadrature(ls, sh.exponents, sh.centers, cls, kernel=kind, omega=omega, ngl=160)
+    assert np.abs(got - ref).max() <= 2e-12 * np.abs(ref).max(), np.abs(got - ref).max() / np.abs(ref).max()
+
+
+def test_attenuated_kernels_sum_and_limits(coulomb_after):
+    """erf + erfc = Coulomb element by element; omega -> infinity: erf -> Coulomb, erfc -> 0; omega -> 0: erf -> 0
+    like omega (2/sqrt pi) omega times the overlap-type integral, checked as a ratio of two small omegas."""
+    rng = np.random.default_rng(92)
+    sh = _rand_shells(rng, [3, 2, 2, 1], K=(2, 1, 1, 2))
+    oracle.set_kernel("coulomb")
+    c = oracle.quartet(sh, 0, 1, 2, 3, quad=True)
+    oracle.set_kernel("erf", 0.45)
+    e = oracle.quartet(sh, 0, 1, 2, 3, quad=True)
+    oracle.set_kernel("erfc", 0.45)
+    ec = oracle.quartet(sh, 0, 1, 2, 3, quad=True)
+    scale = np.abs(c).max()
+    assert np.abs(e + ec - c).max() <= 1e-17 * scale
+    assert np.abs(e).max() > 1e-3 * scale and np.abs(ec).max() > 1e-3 * scale      # both parts matter at this omega
+    oracle.set_kernel("erf", 1e6)
+    assert np.abs(oracle.quartet(sh, 0, 1, 2, 3, quad=True) - c).max() <= 1e-10 * scale
+    oracle.set_kernel("erf", 1e-5)
+    a = oracle.quartet(sh, 0, 1, 2, 3, quad=True)
+    oracle.set_kernel("erf", 2e-5)
+    b = oracle.quartet(sh, 0, 1, 2, 3, quad=True)
+    big = np.abs(a) > 1e-3 * np.abs(a).max()
+    assert np.abs(b[big] / a[big] - 2.0).max() <= 1e-6      # next order: omega^2 r12^2
