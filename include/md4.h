@@ -78,6 +78,16 @@ const char* md4_last_error(const md4_ctx* ctx);
 md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, const int* l,
                           const int* prim_offset, const double* exponents, const double* coefficients);
 
+/* Interaction kernel g(r12) of every later md4_compute / md4_compute_host / md4_debug_hermite_r on this context
+ * (Eq.10: the seed [0]^(m) "is related to the Boys function F_m(x) (or similar quantities for non-Coulomb
+ * integrals)", ref. 21; S:8(f) item 3).  Only the seeds change: G_m = F_m(T) for the Coulomb kernel,
+ * s^(2m+1) F_m(s^2 T) with s^2 = omega^2/(omega^2 + rho) for erf(omega r12)/r12, and their difference for
+ * erfc(omega r12)/r12; the recurrence Eq.13 and both contractions are the same.  omega (1/bohr) must be > 0 and finite
+ * for the attenuated kernels and is ignored for MD4_KERNEL_COULOMB.  Pair lists are kernel-independent.  A launch uses
+ * the kernel that is set when it is enqueued. */
+typedef enum { MD4_KERNEL_COULOMB = 0, MD4_KERNEL_ERF = 1, MD4_KERNEL_ERFC = 2 } md4_kernel;
+md4_status md4_set_kernel(md4_ctx* ctx, int kind, double omega);
+
 /* Shell-pair precompute (S:8(a) a1; Eq.3-5, Eq.16, Listing 2.1 lines 2-3):
  * for every listed ordered pair (i,j) and every primitive pair (ka,kb) computes zeta_p, R_p,
  * ln K_ab = -zeta_a zeta_b/zeta_p |AB|^2 and the matrix H (solid-harmonic pair index x Hermite index)

@@ -281,6 +281,17 @@ md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, c
     return MD4_OK;
 }
 
+md4_status md4_set_kernel(md4_ctx* ctx, int kind, double omega) {
+    if (!ctx) return MD4_EINVAL;
+    if (kind == MD4_KERNEL_COULOMB) { ctx->kernel = {1.0, 0.0, 1.0}; return MD4_OK; }
+    if (kind != MD4_KERNEL_ERF && kind != MD4_KERNEL_ERFC) return fail(ctx, MD4_EINVAL, "md4_set_kernel: unknown kernel");
+    if (!(omega > 0.0) || !std::isfinite(omega) || !std::isfinite(omega * omega))
+        return fail(ctx, MD4_EINVAL, "md4_set_kernel: omega must be > 0 and finite");
+    if (kind == MD4_KERNEL_ERF) ctx->kernel = {0.0, 1.0, omega * omega};
+    else ctx->kernel = {1.0, -1.0, omega * omega};
+    return MD4_OK;
+}
+
 md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** out) {
     if (!ctx) return MD4_EINVAL;
     if (!out) return fail(ctx, MD4_EINVAL, "md4_build_pairs: out is NULL");

@@ -41,6 +41,22 @@ __device__ __forceinline__ void r_tables_to_smem(uint32_t* srt, uint16_t* sad, c
     }
 }
 
+// Interaction kernel g(r12) ("[0]^(m) is related to the Boys function (or similar quantities for non-Coulomb
+// integrals, ref. 21)"; S:8(f) item 3).  For g(r) = Int w(u) exp(-u^2 r^2) du only the seeds of Eq.10 change:
+//   [0]^(m) = (-2 rho)^m prefactor G_m,  G_m = ka F_m(T) + kb s^(2m+1) F_m(s^2 T),  s^2 = omega^2 / (omega^2 + rho):
+//   1/r: (ka, kb) = (1, 0);  erf(omega r)/r: (0, 1);  erfc(omega r)/r: (1, -1).  Everything downstream (Eq.13, the two
+// contractions) is unchanged.
+__device__ __forceinline__ double kernel_seed(const double* __restrict__ boys, const KernelSpec& ks, int m, double rho, double T) {
+    double G = ks.ka != 0.0 ? ks.ka * boys_one(boys, m, T) : 0.0;
+    if (ks.kb != 0.0) {
+        const double s2 = ks.omega2 / (ks.omega2 + rho);
+        double sp = sqrt(s2);
+        for (int k = 0; k < m; ++k) sp *= s2;
+        G = fma(ks.kb * sp, boys_one(boys, m, s2 * T), G);
+    }
+    return G;
+}
+
 // ---- Hermite Coulomb tensor, built by ONE warp in graded order, in place ---------------------------
 // hermite_r_warp computes R^{(0)}_{tuv}, t+u+v <= L, of one primitive quartet into G[graded ordinal]
 // (G: n_hermite(L) + L doubles, sS: 32 doubles; shared memory).  As in Listing 3.1 one array
@@ -57,7 +73,7 @@ __host__ __device__ inline int r_graded_alloc(int L) { return n_hermite(L) + L; 
 
 template <class Poll>
 __device__ __forceinline__ void hermite_r_warp(double* G, double* sS, const uint32_t* srt,
-                                               const double* __restrict__ boys, int L, double zp, double Px,
+                                               const double* __restrict__ boys, const KernelSpec& ks, int L, double zp, double Px,
                                                double Py, double Pz, double zq, double Qx, double Qy, double Qz,
                                                double scale, int lane, Poll poll) {
     const double X0 = Px - Qx, X1 = Py - Qy, X2 = Pz - Qz;
@@ -68,7 +84,7 @@ __device__ __forceinline__ void hermite_r_warp(double* G, double* sS, const uint
         // 2 pi^{5/2} = 34.98683665524972497
         const double pref = scale * 34.986836655249724970 / (zp * zq * sqrt(zs));
         if (lane <= L) {
-            const double F = boys_one(boys, lane, T);
+            const double F = kernel_seed(boys, ks, lane, rho, T);
             double pw = pref;
             const double m2r = -2.0 * rho;
             for (int k = 0; k < lane; ++k) pw *= m2r;

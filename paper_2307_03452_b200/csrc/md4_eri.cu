@@ -46,6 +46,7 @@ struct EriArgs {
     int qmajor;   // 1: a CTA takes whole quartets (items of unequal size); 0: the items of a quartet go to neighbouring CTAs
     int tb;       // bra pairs per strip of the quartet order (quartet_pairs)
     const uint32_t* rtab; const uint32_t* tuv; const double* boys;
+    KernelSpec ks;   // interaction kernel (md4_set_kernel)
     double* tacc;   // [grid][wpc][ncb_q][32][2] partial [ab|q~] of contracted bras
     const uint32_t* colp; const uint32_t* colq;   // bra-order columns of the bra class, ket-order columns of the ket class
     double* out;
@@ -279,7 +280,7 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
         quartet_pairs(a, it, ib, jk);
         const double* sp = a.sb + ((size_t)ib * a.Kb + p) * 8;
         const double* sq = a.sk + ((size_t)jk * a.Kk + q) * 8;
-        hermite_r_warp(GA, sS, srt, a.boys, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
+        hermite_r_warp(GA, sS, srt, a.boys, a.ks, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
                        __ldg(sq + 1), __ldg(sq + 2), __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), lane, poll);
     };
 
@@ -508,6 +509,7 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     }
     a.nst = 2;
     a.rtab = ctx->tab.rtab; a.tuv = ctx->tab.tuv; a.boys = ctx->tab.boys;
+    a.ks = ctx->kernel;
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];
     a.out = d_out;
     a.tacc = ctx->d_tacc;
@@ -537,8 +539,8 @@ __global__ void debug_boys_kernel(const double* tab, int mmax, int n, const doub
 }
 
 // out: dense [(L+1)^3] array, out[(t*(L+1)+u)*(L+1)+v] = R_{tuv} for t+u+v <= L, 0 elsewhere; one warp
-__global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const double* boys, int L, const double* pq,
-                               double* out) {
+__global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const double* boys, KernelSpec ks, int L,
+                               const double* pq, double* out) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int S = L + 1;
     double* Ra = reinterpret_cast<double*>(smem);
@@ -549,7 +551,7 @@ __global__ void debug_r_kernel(const uint32_t* rtab, const uint32_t* tuv, const 
     for (int i = threadIdx.x; i < r_alloc(L); i += blockDim.x) Ra[i] = 0.0;
     r_tables_to_smem(srt, sad, rtab, tuv, L, threadIdx.x, blockDim.x);
     __syncthreads();
-    hermite_r_warp(GA, sS, srt, boys, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7], 1.0, threadIdx.x, [] {});
+    hermite_r_warp(GA, sS, srt, boys, ks, L, pq[0], pq[1], pq[2], pq[3], pq[4], pq[5], pq[6], pq[7], 1.0, threadIdx.x, [] {});
     __syncthreads();
     r_scatter(Ra, GA, sad, L, threadIdx.x, blockDim.x);
     __syncthreads();
@@ -571,7 +573,7 @@ cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_ou
     const size_t sm = ((size_t)r_alloc(L) + 2 * (size_t)n_hermite(L) + 32) * 8 + (size_t)n_hermite(L) * 6 + 16;
     cudaError_t e = cudaFuncSetAttribute(debug_r_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin);
     if (e != cudaSuccess) return e;
-    debug_r_kernel<<<1, 32, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, L, d_pq, d_out);
+    debug_r_kernel<<<1, 32, sm>>>(ctx->tab.rtab, ctx->tab.tuv, ctx->tab.boys, ctx->kernel, L, d_pq, d_out);
     ctx->launches++;
     return cudaGetLastError();
 }

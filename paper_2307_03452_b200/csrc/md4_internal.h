@@ -96,6 +96,11 @@ struct PairListDev {
     int* ij;             // [npair*2]
 };
 
+// Interaction kernel (md4_device.cuh kernel_seed): G_m = ka F_m(T) + kb s^(2m+1) F_m(s^2 T), s^2 = omega2/(omega2 + rho)
+struct KernelSpec {
+    double ka, kb, omega2;
+};
+
 // One device allocation that the context may hand from a released pair list to the next one of (about) that size.
 // ev (may be null) completes when the last kernel that touches the block has finished; whoever reuses the block
 // makes its first writer wait for it (stream-ordered, the host never blocks).
@@ -158,6 +163,7 @@ struct md4_ctx {
     static constexpr int NSLICE_EV = 8;   // md4_compute_host: bra slices whose D2H copy overlaps the next slice's kernel
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t slice_ev[NSLICE_EV] = {};
+    md4::KernelSpec kernel = {1.0, 0.0, 1.0};   // interaction kernel of md4_compute: 1/r12 unless md4_set_kernel changed it
     long long launches = 0;
     int num_sms = 0;
     int smem_optin = 0;

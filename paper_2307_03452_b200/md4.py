@@ -15,12 +15,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmd4.so")
 
 MD4_OK, MD4_EINVAL, MD4_EUNSUPPORTED, MD4_ESTATE, MD4_ENOMEM, MD4_ECUDA = range(6)
+KERNELS = {"coulomb": 0, "erf": 1, "erfc": 2}   # md4_kernel of include/md4.h
 STATUS_NAMES = ["MD4_OK", "MD4_EINVAL", "MD4_EUNSUPPORTED", "MD4_ESTATE", "MD4_ENOMEM", "MD4_ECUDA"]
 
 #: every symbol include/md4.h declares (tests check the library exports exactly these)
 SYMBOLS = [
     "md4_create", "md4_destroy", "md4_last_error", "md4_set_shells", "md4_build_pairs", "md4_free_pairs",
-    "md4_stream_wait_pairs",
+    "md4_stream_wait_pairs", "md4_set_kernel",
     "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host",
     "md4_launch_count", "md4_flops_per_quartet", "md4_debug_boys", "md4_debug_solid_coeff",
     "md4_debug_hermite_r", "md4_debug_pair_h", "md4_debug_work_items",
@@ -57,6 +58,8 @@ def load():
     lib.md4_build_pairs.restype = ctypes.c_int
     lib.md4_free_pairs.argtypes = [vp, vp]
     lib.md4_free_pairs.restype = None
+    lib.md4_set_kernel.argtypes = [vp, ctypes.c_int, ctypes.c_double]
+    lib.md4_set_kernel.restype = ctypes.c_int
     lib.md4_stream_wait_pairs.argtypes = [vp, vp, vp]
     lib.md4_stream_wait_pairs.restype = ctypes.c_int
     lib.md4_pairs_count.argtypes = [vp]
@@ -166,6 +169,10 @@ class Engine:
         ex = np.ascontiguousarray(exponents, dtype=np.float64)
         co = np.ascontiguousarray(coefficients, dtype=np.float64)
         self._check(load().md4_set_shells(self.handle, int(li.shape[0]), _dp(c), _ip(li), _ip(off), _dp(ex), _dp(co)))
+
+    def set_kernel(self, kind: str = "coulomb", omega: float = 0.0):
+        """Interaction kernel of later compute calls: "coulomb" (1/r12), "erf" or "erfc" (attenuated with omega)."""
+        self._check(load().md4_set_kernel(self.handle, KERNELS[kind], float(omega)))
 
     def build_pairs(self, ij) -> PairList:
         a = np.ascontiguousarray(ij, dtype=np.int32).reshape(-1, 2)

@@ -13,8 +13,10 @@ import numpy as np
 import oracle
 
 
-def mp_R_dict(L, zp, P, zq, Q):
-    """{(t,u,v): R^{(0)}_{tuv}} as mpmath numbers, t+u+v <= L; prefactor 2 pi^{5/2}/(zp zq sqrt(zp+zq)) included."""
+def mp_R_dict(L, zp, P, zq, Q, kernel="coulomb", omega=None):
+    """{(t,u,v): R^{(0)}_{tuv}} as mpmath numbers, t+u+v <= L; prefactor 2 pi^{5/2}/(zp zq sqrt(zp+zq)) included.
+    kernel "erf" / "erfc": seeds from the truncated Boys integral Int y^2m exp(-T y^2) dy over [0, s] / [s, 1],
+    s^2 = omega^2/(omega^2 + rho), by mpmath quadrature of that definition (ref. 21)."""
     import mpmath as mp
 
     mp.mp.dps = 40
@@ -25,6 +27,10 @@ def mp_R_dict(L, zp, P, zq, Q):
     pref = 2 * mp.pi ** mp.mpf(2.5) / (zp * zq * mp.sqrt(zp + zq))
 
     def F(m):
+        if kernel != "coulomb":
+            s = mp.sqrt(mp.mpf(omega) ** 2 / (mp.mpf(omega) ** 2 + rho))
+            lo, hi = (0, s) if kernel == "erf" else (s, 1)
+            return mp.quad(lambda y: y ** (2 * m) * mp.exp(-T * y * y), [lo, hi])
         if T == 0:
             return mp.mpf(1) / (2 * m + 1)
         return mp.gammainc(m + mp.mpf(1) / 2, 0, T) / (2 * T ** (m + mp.mpf(1) / 2))
@@ -48,9 +54,9 @@ def mp_R_dict(L, zp, P, zq, Q):
     return {k[1:]: val for k, val in R.items() if k[0] == 0}
 
 
-def mp_R(L, zp, P, zq, Q):
+def mp_R(L, zp, P, zq, Q, kernel="coulomb", omega=None):
     """R^{(0)}_{tuv} as a float array [L+1]^3 (entries with t+u+v > L are 0)."""
-    R = mp_R_dict(L, zp, [float(x) for x in P], zq, [float(x) for x in Q])
+    R = mp_R_dict(L, zp, [float(x) for x in P], zq, [float(x) for x in Q], kernel, omega)
     out = np.zeros((L + 1,) * 3)
     for (t, u, v), val in R.items():
         out[t, u, v] = float(val)

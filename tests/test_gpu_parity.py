@@ -442,3 +442,64 @@ def test_repeated_launches_are_bit_identical(eng, which):
         torch.cuda.synchronize()
         assert torch.equal(out, ref), f"{which}: launch {rep + 2} differs from the first in {int((out != ref).sum())} elements"
     bra.free(); ket.free()
+
+
+# ------------------------------------------------------------------- non-Coulomb kernels (S:8(f) item 3)
+@pytest.fixture
+def coulomb_after(eng):
+    yield
+    eng.set_kernel("coulomb")
+    oracle.set_kernel("coulomb")
+
+
+@pytest.mark.parametrize("kind,omega", [("erf", 0.4), ("erfc", 0.4), ("erfc", 2.5)])
+def test_attenuated_kernel_r_stage(eng, coulomb_after, kind, omega):
+    """R^{(0)}_{tuv} with the seeds of erf(omega r)/r and erfc(omega r)/r: device (table Boys at T and s^2 T) vs a
+    40-digit recursion seeded by mpmath quadrature of the truncated Boys integral."""
+    eng.set_kernel(kind, omega)
+    for L, zp, zq, P, Q in [(16, 1.7, 0.9, (0.1, 0.2, -0.3), (1.0, -0.7, 0.45)), (12, 0.3, 0.2, (1.0, 1.0, 1.0), (1.0, 1.0, 1.0)),
+                            (10, 30.0, 45.0, (0.0, 0.0, 0.0), (1.5, 2.0, 2.5))]:
+        got = eng.debug_hermite_r(L, zp, P, zq, Q)
+        ref = _mp_R(L, zp, P, zq, Q, kind, omega)
+        # the Coulomb R of the same primitive quartet sets the scale (erfc is a difference of two such tensors)
+        scale = _mp_R(L, zp, P, zq, Q)
+        for n in range(L + 1):
+            idx = [(t, u, n - t - u) for t in range(n + 1) for u in range(n - t + 1)]
+            r = np.array([ref[i] for i in idx]); g = np.array([got[i] for i in idx]); sc = np.array([scale[i] for i in idx])
+            assert np.abs(g - r).max() <= _r_stage_tol(n) * max(np.abs(r).max(), np.abs(sc).max()), (kind, L, n)
+
+
+@pytest.mark.parametrize("kind,omega", [("erf", 0.35), ("erfc", 0.35), ("erfc", 1.5)])
+@pytest.mark.parametrize("lclass,kclass", [((2, 1, 1, 0), (1, 2, 1, 1)), ((4, 4, 4, 4), (1, 1, 1, 1)), ((6, 5, 5, 4), (1, 1, 1, 1)),
+                                           ((6, 6, 6, 6), (1, 1, 1, 1)), ((6, 6, 6, 6), (2, 1, 1, 2))])
+def test_attenuated_kernels_end_to_end(eng, coulomb_after, kind, omega, lclass, kclass):
+    """(ab|cd) with erf(omega r12)/r12 and erfc(omega r12)/r12 through the whole path against the binary128 oracle with the
+    same kernel; bar 1e-10 of the quartet's maximum."""
+    wl = inputs.small_workload(lclass, kclass, nbra=3, nket=2, seed=41)
+    eng.set_kernel(kind, omega)
+    oracle.set_kernel(kind, omega)
+    g, r = _run(eng, wl)
+    errs, below = _quartet_errors(g, r)
+    assert errs.max() <= TOL, (kind, omega, lclass, errs.max())
+
+
+def test_attenuated_kernels_add_up_on_the_gpu(eng, coulomb_after):
+    """erf + erfc = Coulomb on a full-size launch (cfg2, 4096 (hh|hh) quartets): every element, to rounding."""
+    import torch
+
+    wl = inputs.config2()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    c = eng.compute(bra, ket).clone()
+    eng.set_kernel("erf", 0.5)
+    e = eng.compute(bra, ket).clone()
+    eng.set_kernel("erfc", 0.5)
+    ec = eng.compute(bra, ket)
+    torch.cuda.synchronize()
+    scale = c.abs().amax(dim=(2, 3, 4, 5), keepdim=True)
+    assert ((e + ec - c).abs() / scale).max() <= 1e-11
+    assert (e.abs() / scale).max() > 1e-2 and (ec.abs() / scale).max() > 1e-2
+    with pytest.raises(Exception):
+        eng.set_kernel("erf", -1.0)
+    bra.free(); ket.free()
