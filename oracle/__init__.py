@@ -192,3 +192,42 @@ def compute(sh: Shells, bra_ij, ket_ij, subset=None, nthreads: int | None = None
     if rc:
         raise RuntimeError(f"oracle_compute failed rc={rc}")
     return out
+
+
+def ao_offsets(sh: Shells) -> np.ndarray:
+    """First AO (solid-harmonic function) of every shell and the total: shells in table order, 2l+1 functions each,
+    m = -l..+l ascending -- the AO order md4_compute_jk uses (include/md4.h)."""
+    return np.concatenate([[0], np.cumsum(2 * sh.l.astype(np.int64) + 1)])
+
+
+def digest_jk(sh: Shells, bra_ij, ket_ij, D, **kw):
+    """Direct digestion of a (bra list x ket list) batch into Coulomb- and exchange-type matrices ("computing
+    Fock matrix elements directly", :249), written out as its definition: for EVERY listed quartet
+    (bra pair (a,b), ket pair (c,d)), exactly
+
+        J[a, b] += sum_{cd} (ab|cd) D[c, d]          K[a, c] += sum_{bd} (ab|cd) D[b, d]
+
+    over the AO blocks of the four shells; nothing else (no permutational images, no factors: the caller lists what it
+    wants).  Integrals from compute() (binary128 by default, rounded to double), contraction and accumulation in long
+    double.  Returns (J, K) as long-double [nbf, nbf] arrays."""
+    off = ao_offsets(sh)
+    nbf = int(off[-1])
+    Dl = np.asarray(D, dtype=np.longdouble).reshape(nbf, nbf)
+    bra = np.ascontiguousarray(bra_ij, dtype=np.int32).reshape(-1, 2)
+    ket = np.ascontiguousarray(ket_ij, dtype=np.int32).reshape(-1, 2)
+    J = np.zeros((nbf, nbf), dtype=np.longdouble)
+    K = np.zeros((nbf, nbf), dtype=np.longdouble)
+    if bra.shape[0] == 0 or ket.shape[0] == 0:
+        return J, K
+    eri = compute(sh, bra, ket, **kw).astype(np.longdouble)      # [i, j, ma, mb, mc, md]
+    for i, (a, b) in enumerate(bra):
+        sa, sb = slice(off[a], off[a + 1]), slice(off[b], off[b + 1])
+        for j, (c, d) in enumerate(ket):
+            sc, sd = slice(off[c], off[c + 1]), slice(off[d], off[d + 1])
+            g = eri[i, j]
+            for ma in range(g.shape[0]):
+                for mb in range(g.shape[1]):
+                    J[off[a] + ma, off[b] + mb] += (g[ma, mb] * Dl[sc, sd]).sum()
+                    for mc in range(g.shape[2]):
+                        K[off[a] + ma, off[c] + mc] += (g[ma, mb, mc, :] * Dl[off[b] + mb, sd]).sum()
+    return J, K

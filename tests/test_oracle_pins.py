@@ -450,3 +450,55 @@ def test_attenuated_kernels_sum_and_limits(coulomb_after):
     b = oracle.quartet(sh, 0, 1, 2, 3, quad=True)
     big = np.abs(a) > 1e-3 * np.abs(a).max()
     assert np.abs(b[big] / a[big] - 2.0).max() <= 1e-6      # next order: omega^2 r12^2
+
+
+# ------------------------------------------------ direct digestion
+def test_digest_jk_hand_computed_s_shells():
+    """Four s shells, bra list [(0,1),(2,0)], ket list [(2,3),(1,1)]: J and K by hand from the closed form
+    (ss|ss) = K_ab K_cd 2 pi^{5/2}/(p q sqrt(p+q)) F_0(T), F_0 = sqrt(pi/T) erf(sqrt T)/2 (math.erf), summed quartet by
+    quartet in this test -- not by the oracle's contraction code."""
+    rng = np.random.default_rng(5)
+    cent = rng.uniform(0, 2.0, (4, 3))
+    ex = np.array([0.8, 1.3, 0.5, 2.1])
+    co = np.array([0.7, 1.1, 0.9, 0.6])
+    sh = oracle.Shells(cent, [0, 0, 0, 0], [0, 1, 2, 3, 4], ex, co)
+    D = rng.uniform(-1, 1, (4, 4))
+    bra, ket = [(0, 1), (2, 0)], [(2, 3), (1, 1)]
+
+    def ssss(a, b, c, d):
+        p, q = ex[a] + ex[b], ex[c] + ex[d]
+        P = (ex[a] * cent[a] + ex[b] * cent[b]) / p
+        Q = (ex[c] * cent[c] + ex[d] * cent[d]) / q
+        kab = math.exp(-ex[a] * ex[b] / p * ((cent[a] - cent[b]) ** 2).sum())
+        kcd = math.exp(-ex[c] * ex[d] / q * ((cent[c] - cent[d]) ** 2).sum())
+        T = p * q / (p + q) * ((P - Q) ** 2).sum()
+        f0 = 1.0 if T == 0 else 0.5 * math.sqrt(math.pi / T) * math.erf(math.sqrt(T))
+        return co[a] * co[b] * co[c] * co[d] * kab * kcd * 2 * math.pi ** 2.5 / (p * q * math.sqrt(p + q)) * f0
+
+    Jh, Kh = np.zeros((4, 4)), np.zeros((4, 4))
+    for a, b in bra:
+        for c, d in ket:
+            v = ssss(a, b, c, d)
+            Jh[a, b] += v * D[c, d]
+            Kh[a, c] += v * D[b, d]
+    J, K = oracle.digest_jk(sh, bra, ket, D)
+    assert np.abs(J.astype(float) - Jh).max() <= 1e-14 * np.abs(Jh).max()
+    assert np.abs(K.astype(float) - Kh).max() <= 1e-14 * np.abs(Kh).max()
+    assert np.count_nonzero(Jh) == 2 and np.count_nonzero(Kh) == 4      # only the listed blocks are touched
+
+
+def test_digest_jk_index_roles_with_unit_densities():
+    """(dp|pd)-type shells with a density that is 1 in ONE element: J then is one (c,d) slice of the quartet and K one
+    (b,d) slice, taken here straight from oracle.quartet -- a swapped pair of indices in the contraction would fail."""
+    rng = np.random.default_rng(6)
+    sh = _rand_shells(rng, [2, 1, 1, 2])
+    off = oracle.ao_offsets(sh)
+    g = oracle.quartet(sh, 0, 1, 2, 3, quad=True).astype(np.float64)      # [5, 3, 3, 5]
+    nbf = int(off[-1])
+    mc, md, mb = 2, 3, 1
+    D = np.zeros((nbf, nbf)); D[off[2] + mc, off[3] + md] = 1.0
+    J, K = oracle.digest_jk(sh, [(0, 1)], [(2, 3)], D)
+    assert np.array_equal(J[off[0]:off[1], off[1]:off[2]].astype(float), g[:, :, mc, md]) and np.abs(K).max() == 0
+    D = np.zeros((nbf, nbf)); D[off[1] + mb, off[3] + md] = 1.0
+    J, K = oracle.digest_jk(sh, [(0, 1)], [(2, 3)], D)
+    assert np.array_equal(K[off[0]:off[1], off[2]:off[3]].astype(float), g[:, mb, :, md]) and np.abs(J).max() == 0
