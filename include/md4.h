@@ -139,6 +139,31 @@ md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket,
 md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* h_out,
                             size_t capacity_doubles, void* cuda_stream);
 
+/* ---- direct digestion (S:8(f) item 2; "computing Fock matrix elements directly", P:249 exchange matrix) ------
+ * AO order: the shells of md4_set_shells in table order, 2l+1 real solid harmonics each, m = -l..+l ascending;
+ * md4_num_ao gives their number nbf for the current shell set.  A pair list remembers the AO offsets of its shells
+ * (of the shell set it was built from). */
+md4_status md4_num_ao(const md4_ctx* ctx, int* nbf);
+
+/* For EVERY quartet of (bra list) x (ket list) -- bra pair (a,b), ket pair (c,d) -- exactly
+ *     J[a,b] += sum_{cd} (ab|cd) D[c,d]          K[a,c] += sum_{bd} (ab|cd) D[b,d]
+ * over the AO blocks of the four shells, and nothing else: no permutational images, no factors (the caller lists the
+ * quartets it wants and scales D).  The integrals are contracted with the density blocks in the epilogue of the fused
+ * kernel and are never written out: per quartet 8 Nab Ncd bytes of output stream become a few hundred atomic adds.
+ *   d_D      DEVICE [nbf*nbf] row-major, read only
+ *   d_J, d_K DEVICE [nbf*nbf] row-major, ACCUMULATED into (+=, double atomics: the order of the additions, hence the
+ *            last bits, may differ from run to run); either may be NULL (not computed), not both
+ * Same stream semantics as md4_compute (enqueue only).  Empty lists: MD4_OK, nothing touched.  Uses the current
+ * interaction kernel (md4_set_kernel). */
+md4_status md4_compute_jk(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, const double* d_D,
+                          double* d_J, double* d_K, void* cuda_stream);
+
+/* Same through HOST matrices (the end-to-end path of bench.py's "e2e_digest"): copies D and the starting values of
+ * J / K to the device, runs md4_compute_jk, copies J / K back and synchronises.  3 nbf^2 doubles cross the bus instead
+ * of Nab Ncd doubles per quartet. */
+md4_status md4_compute_jk_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, const double* h_D,
+                               double* h_J, double* h_K, void* cuda_stream);
+
 /* Number of kernel launches this context has enqueued so far (bench.py's "gpu_launches"). */
 long long md4_launch_count(const md4_ctx* ctx);
 

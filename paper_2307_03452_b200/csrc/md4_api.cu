@@ -34,7 +34,7 @@ md4_status cuda_fail(md4_ctx* ctx, const char* what, cudaError_t e) {
 // forget the shell set (the device block is kept for the next one); release: the context is going away
 void free_shells(md4_ctx* c, bool release = false) {
     c->d_centers = nullptr; c->d_l = nullptr; c->d_off = nullptr; c->d_exp = nullptr; c->d_coef = nullptr;
-    c->nshell = 0; c->nprim = 0; c->h_l.clear(); c->h_off.clear();
+    c->nshell = 0; c->nprim = 0; c->h_l.clear(); c->h_off.clear(); c->h_ao.clear();
     if (release) {
         cudaFree(c->d_shell_block); c->d_shell_block = nullptr; c->shell_block_bytes = 0;
         if (c->h_shell_stage) cudaFreeHost(c->h_shell_stage);
@@ -278,6 +278,8 @@ md4_status md4_set_shells(md4_ctx* ctx, int nshell, const double* centers_xyz, c
     ctx->nshell = nshell; ctx->nprim = nprim;
     ctx->h_l.assign(l, l + nshell);
     ctx->h_off.assign(prim_offset, prim_offset + nshell + 1);
+    ctx->h_ao.assign((size_t)nshell + 1, 0);
+    for (int i = 0; i < nshell; ++i) ctx->h_ao[i + 1] = ctx->h_ao[i] + n_solid(l[i]);
     return MD4_OK;
 }
 
@@ -331,7 +333,7 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
         auto up = [](size_t x) { return (x + 255) / 256 * 256; };
         const size_t oHb = 0, oHk = oHb + up(nprim * d.hstrideb * sizeof(double)), oSc = oHk + up(nprim * d.hstridek * sizeof(double)),
                      oPm = oSc + up(nprim * 8 * sizeof(double)), oIj = oPm + up((size_t)npair * sizeof(double)),
-                     total = oIj + up((size_t)npair * 2 * sizeof(int));
+                     total = oIj + up((size_t)npair * 4 * sizeof(int));   // ij, then the AO offsets of the same shells
         cudaError_t e = pool_alloc(ctx, total, &pl->block);
         if (e == cudaSuccess) {
             char* base = static_cast<char*>(pl->block.p);
@@ -340,6 +342,8 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
             pl->d.scal = reinterpret_cast<double*>(base + oSc);
             pl->d.pairmax = reinterpret_cast<double*>(base + oPm);
             pl->d.ij = reinterpret_cast<int*>(base + oIj);
+            pl->d.ao = pl->d.ij + 2 * (size_t)npair;
+            pl->d.nbf = ctx->h_ao[ctx->nshell];
             e = cudaEventCreateWithFlags(&pl->ready, cudaEventDisableTiming);
         }
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->last_use, cudaEventDisableTiming);
@@ -355,7 +359,7 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
         if (e == cudaSuccess) {
             const int sl = ctx->stage_next;
             ctx->stage_next = (sl + 1) % md4_ctx::NSTAGE;
-            const size_t n = (size_t)npair * 2;
+            const size_t n = (size_t)npair * 4;
             if (ctx->stage_done[sl]) e = cudaEventSynchronize(ctx->stage_done[sl]);
             else e = cudaEventCreateWithFlags(&ctx->stage_done[sl], cudaEventDisableTiming);
             if (e == cudaSuccess && ctx->stage_ints[sl] < n) {
@@ -366,7 +370,8 @@ md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** o
                 if (e == cudaSuccess) ctx->stage_ints[sl] = cap;
             }
             if (e == cudaSuccess) {
-                std::memcpy(ctx->h_stage[sl], ij, n * sizeof(int));
+                std::memcpy(ctx->h_stage[sl], ij, (size_t)npair * 2 * sizeof(int));
+                for (size_t t = 0; t < (size_t)npair * 2; ++t) ctx->h_stage[sl][(size_t)npair * 2 + t] = ctx->h_ao[ij[t]];
                 e = cudaMemcpyAsync(pl->d.ij, ctx->h_stage[sl], n * sizeof(int), cudaMemcpyHostToDevice, ctx->build_stream);
             }
             if (e == cudaSuccess) e = cudaEventRecord(ctx->stage_done[sl], ctx->build_stream);
@@ -524,6 +529,7 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
         sub.scal += (size_t)b0 * kk * 8;
         sub.pairmax += b0;
         sub.ij += 2 * (size_t)b0;
+        sub.ao += 2 * (size_t)b0;
         double* d_slice = ctx->d_scratch + (size_t)b0 * per_bra;
         s = launch_eri(ctx, sub, ket->d, d_slice, st);
         if (s != MD4_OK) { cudaStreamSynchronize(st); cudaStreamSynchronize(ctx->copy_stream); return s; }
@@ -538,6 +544,79 @@ md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs*
     cudaError_t e3 = cudaStreamSynchronize(ctx->copy_stream);
     if (e == cudaSuccess) e = e2 != cudaSuccess ? e2 : e3;
     if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_host", e);
+    return MD4_OK;
+}
+
+md4_status md4_num_ao(const md4_ctx* ctx, int* nbf) {
+    if (!ctx || !nbf) return MD4_EINVAL;
+    *nbf = ctx->nshell ? ctx->h_ao[ctx->nshell] : 0;
+    return MD4_OK;
+}
+
+static md4_status check_jk(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, const void* D, const void* J, const void* K,
+                           bool* empty) {
+    if (!ctx) return MD4_EINVAL;
+    if (!bra || !ket) return fail(ctx, MD4_EINVAL, "md4_compute_jk: pair list is NULL");
+    if (bra->ctx != ctx || ket->ctx != ctx || !ctx->lists.count(const_cast<md4_pairs*>(bra)) ||
+        !ctx->lists.count(const_cast<md4_pairs*>(ket)))
+        return fail(ctx, MD4_ESTATE, "md4_compute_jk: pair list does not belong to this context");
+    *empty = bra->d.npair == 0 || ket->d.npair == 0;
+    if (*empty) return MD4_OK;
+    if (!D) return fail(ctx, MD4_EINVAL, "md4_compute_jk: density pointer is NULL");
+    if (!J && !K) return fail(ctx, MD4_EINVAL, "md4_compute_jk: J and K are both NULL");
+    if (bra->d.nbf != ket->d.nbf) return fail(ctx, MD4_ESTATE, "md4_compute_jk: the two lists were built from shell sets of different size");
+    if ((((uintptr_t)D) | ((uintptr_t)J) | ((uintptr_t)K)) & 7) return fail(ctx, MD4_EINVAL, "md4_compute_jk: pointer not 8-byte aligned");
+    return MD4_OK;
+}
+
+md4_status md4_compute_jk(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, const double* d_D, double* d_J, double* d_K,
+                          void* cuda_stream) {
+    bool empty = false;
+    md4_status s = check_jk(ctx, bra, ket, d_D, d_J, d_K, &empty);
+    if (s != MD4_OK || empty) return s;
+    DeviceGuard g(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = order_before(ctx, bra, ket, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_jk", e);
+    DigestArgs dg{bra->d.nbf, d_D, d_J, d_K};
+    s = launch_eri(ctx, bra->d, ket->d, nullptr, st, &dg);
+    if (s != MD4_OK) return s;
+    e = order_after(ctx, bra, ket, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_jk", e);
+    return MD4_OK;
+}
+
+md4_status md4_compute_jk_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, const double* h_D, double* h_J, double* h_K,
+                               void* cuda_stream) {
+    bool empty = false;
+    md4_status s = check_jk(ctx, bra, ket, h_D, h_J, h_K, &empty);
+    if (s != MD4_OK || empty) return s;
+    DeviceGuard g(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n2 = (size_t)bra->d.nbf * bra->d.nbf;
+    const size_t need = 3 * n2;   // D | J | K
+    if (ctx->scratch_doubles < need) {
+        cudaFree(ctx->d_scratch);
+        ctx->d_scratch = nullptr; ctx->scratch_doubles = 0;
+        void* t = nullptr;
+        cudaError_t e = ctx_malloc(ctx, &t, need * sizeof(double));
+        if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_jk_host", e);
+        ctx->d_scratch = static_cast<double*>(t);
+        ctx->scratch_doubles = need;
+    }
+    double *dD = ctx->d_scratch, *dJ = dD + n2, *dK = dJ + n2;
+    cudaError_t e = cudaMemcpyAsync(dD, h_D, n2 * sizeof(double), cudaMemcpyHostToDevice, st);
+    // J and K ACCUMULATE (+=): the host values are the starting point
+    if (e == cudaSuccess && h_J) e = cudaMemcpyAsync(dJ, h_J, n2 * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && h_K) e = cudaMemcpyAsync(dK, h_K, n2 * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_jk_host", e);
+    s = md4_compute_jk(ctx, bra, ket, dD, h_J ? dJ : nullptr, h_K ? dK : nullptr, cuda_stream);
+    if (s != MD4_OK) { cudaStreamSynchronize(st); return s; }
+    if (h_J) e = cudaMemcpyAsync(h_J, dJ, n2 * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h_K) e = cudaMemcpyAsync(h_K, dK, n2 * sizeof(double), cudaMemcpyDeviceToHost, st);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = e2;
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_jk_host", e);
     return MD4_OK;
 }
 

@@ -50,6 +50,11 @@ struct EriArgs {
     double* tacc;   // [grid][wpc][ncb_q][32][2] partial [ab|q~] of contracted bras
     const uint32_t* colp; const uint32_t* colq;   // bra-order columns of the bra class, ket-order columns of the ket class
     double* out;
+    // direct digestion (md4_compute_jk): instead of storing (ab|cd), J[a,b] += sum_cd (ab|cd) D[c,d] and
+    // K[a,c] += sum_bd (ab|cd) D[b,d] on AO matrices [nbf x nbf]; aob / aok = AO offsets of the shells of every pair
+    int digest, nbf, nsb, nsd;        // nsb = 2 l_b + 1, nsd = 2 l_d + 1
+    const int* aob; const int* aok;
+    const double* D; double* J; double* K;
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -57,8 +62,10 @@ __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a -
 // Shared memory: R in the additive layout | H_cd ring | graded R of the next primitive quartet (GA) | seeds | gather offsets of the p~ and q~ columns | sign bits | Eq.13 table |
 // additive address per graded ordinal | mbarriers.
 struct SmemLayout {
-    size_t ra, un, ga, ss, ap, aq, sg, rt, ad, bars, total, stage_bytes;
-    __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst) {
+    size_t ra, un, ga, ss, ap, aq, sg, rt, ad, bars, dg, total, stage_bytes;
+    // digest: D_cd of the ket pair (padded to whole column blocks), D_bd, the K_ac tile of the item, column -> (mc, md)
+    static constexpr int DG_TILE = (2 * LMAX + 1) * (2 * LMAX + 1);
+    __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst, int digest = 0) {
         size_t o = 0;
         ra = o; o += align_up((size_t)r_alloc(L) * 8, 128);
         stage_bytes = (size_t)nrb_cd * 64 * 8;
@@ -71,6 +78,8 @@ struct SmemLayout {
         rt = o; o += align_up((size_t)n_hermite(L) * 4, 16);   // Eq.13 table
         ad = o; o += align_up((size_t)n_hermite(L) * 2, 16);   // additive address per graded ordinal
         bars = o; o += 2 * MAX_STAGES * 8;
+        dg = o;
+        if (digest) o += (size_t)nrb_cd * 64 + 2 * DG_TILE * 8 + align_up((size_t)nrb_cd * 8 * 2, 16);
         total = o;
     }
 };
@@ -211,7 +220,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
 template <int NT_CD, int NQT, int MAXW, bool EXACT, int MINB>
 __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
-    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst);
+    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst, a.digest);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
     double* GA = reinterpret_cast<double*>(smem + lay.ga);
     double* sS = reinterpret_cast<double*>(smem + lay.ss);
@@ -222,6 +231,10 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     uint16_t* sad = reinterpret_cast<uint16_t*>(smem + lay.ad);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + lay.bars);
     uint64_t* empty = full + MAX_STAGES;
+    double* sDcd = reinterpret_cast<double*>(smem + lay.dg);          // [nrb_cd * 8]
+    double* sDbd = sDcd + a.nrb_cd * 8;                               // [nsb * nsd]
+    double* sK = sDbd + SmemLayout::DG_TILE;                          // [nsa * nsc]
+    uint16_t* cmap = reinterpret_cast<uint16_t*>(sK + SmemLayout::DG_TILE);   // column of cd -> mc << 8 | md
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const int L = a.L;
@@ -246,6 +259,10 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
             if (!(q & COL_PAD)) m |= (((q & 255) + ((q >> 8) & 255) + ((q >> 16) & 255)) & 1u) << c;
         }
         sg[b] = m;
+    }
+    if (a.digest) {
+        for (int c = tid; c < a.nrb_cd * 8; c += nthr) cmap[c] = (uint16_t)(c < a.ncd ? ((c / a.nsd) << 8) | (c % a.nsd) : 0);
+        for (int c = tid; c < SmemLayout::DG_TILE; c += nthr) sK[c] = 0.0;
     }
     if (tid == 0) {
         for (int s = 0; s < a.nst; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)a.wpc); }
@@ -294,6 +311,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     if (have && producer) build_r(quartet, 0, 0, [] {});
 
     double2 acc[NT_CD];
+    int k_ao_a = 0, k_ao_c = 0;     // digest: AO offsets of the K tile being accumulated in shared memory
+    bool k_pending = false;
     while (have) {
         long long nquartet = quartet;
         int nms = ms, nkq = kq, nkp = kp + 1;
@@ -323,6 +342,24 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
         }
         __syncthreads();  // consumers are done with R of the previous primitive quartet, the builder with GA
         r_scatter(Ra, GA, sad, L, tid, nthr);
+        if (a.digest && kq == 0 && kp == 0) {
+            // a new item: the K tile of the previous one goes to the AO matrix (global atomics), then the density blocks
+            // of this quartet are staged: D_cd (for J) and D_bd (for K)
+            const int nsa = a.nab / a.nsb, nsc = a.ncd / a.nsd;
+            if (k_pending) {
+                for (int e = tid; e < nsa * nsc; e += nthr) {
+                    const double v = sK[e];
+                    sK[e] = 0.0;
+                    if (v != 0.0) atomicAdd(a.K + (size_t)(k_ao_a + e / nsc) * a.nbf + k_ao_c + e % nsc, v);
+                }
+            }
+            const int ao_b = __ldg(a.aob + 2 * ib + 1), ao_c = __ldg(a.aok + 2 * jk), ao_d = __ldg(a.aok + 2 * jk + 1);
+            for (int c = tid; c < a.nrb_cd * 8; c += nthr)
+                sDcd[c] = c < a.ncd ? __ldg(a.D + (size_t)(ao_c + c / a.nsd) * a.nbf + ao_d + c % a.nsd) : 0.0;
+            for (int e = tid; e < a.nsb * a.nsd; e += nthr)
+                sDbd[e] = __ldg(a.D + (size_t)(ao_b + e / a.nsd) * a.nbf + ao_d + e % a.nsd);
+            k_ao_a = __ldg(a.aob + 2 * ib); k_ao_c = ao_c; k_pending = true;
+        }
         __syncthreads();
 
         const bool last_kp = (kp == a.Kb - 1);   // the ket transform (and the ring) run with the last bra primitive only
@@ -372,7 +409,43 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
             // ---- epilogue after the last primitive quartet of the item: common factor K_ab K_cd of the pair
             // maxima, applied in two halves so that results near the bottom of the FP64 range are still
             // correctly rounded
-            if (item_ends) {
+            if (item_ends && a.digest) {
+                // ---- direct digestion: the row's (ab|cd) values meet D_cd (Coulomb-type J, one number per
+                // row after a reduction over the four lanes of the row) and D_bd (exchange-type K, accumulated per (ma, mc)
+                // in the shared-memory tile); nothing is stored per quartet
+                const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
+                const int row = mbk * 8 + (lane >> 2);
+                const bool rowok = row < a.nab;
+                const int ma = rowok ? row / a.nsb : 0, mb = rowok ? row % a.nsb : 0;
+                const int nsc = a.ncd / a.nsd;
+                double js = 0.0, ks = 0.0;
+                int cur = -1;
+#pragma unroll
+                for (int nb = 0; nb < NT_CD; ++nb) {
+                    const int col = nb * 8 + 2 * cc.k4;
+                    const double vx = (acc[nb].x * f) * f, vy = (acc[nb].y * f) * f;
+                    js = fma(vx, sDcd[col], fma(vy, sDcd[col + 1], js));
+                    if (a.K) {
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const int c = col + h;
+                            if (c < a.ncd && rowok) {
+                                const int w = cmap[c], mc = w >> 8, md = w & 255;
+                                if (mc != cur) {
+                                    if (cur >= 0) atomicAdd(sK + ma * nsc + cur, ks);
+                                    cur = mc; ks = 0.0;
+                                }
+                                ks = fma(h ? vy : vx, sDbd[mb * a.nsd + md], ks);
+                            }
+                        }
+                    }
+                }
+                if (a.K && cur >= 0) atomicAdd(sK + ma * nsc + cur, ks);
+                js += __shfl_xor_sync(0xffffffffu, js, 1);
+                js += __shfl_xor_sync(0xffffffffu, js, 2);
+                if (a.J && rowok && cc.k4 == 0)
+                    atomicAdd(a.J + (size_t)(__ldg(a.aob + 2 * ib) + ma) * a.nbf + __ldg(a.aob + 2 * ib + 1) + mb, js);
+            } else if (item_ends) {
                 const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
                 const int row = mbk * 8 + (lane >> 2);
                 // (a9) 16-byte streaming stores (st.global.cs.v2.f64: the 3.7 GB output stream must not evict H from L2).
@@ -406,6 +479,14 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
         }
         quartet = nquartet; ms = nms; kq = nkq; kp = nkp; have = nhave;
     }
+    if (a.digest && k_pending) {
+        __syncthreads();
+        const int nsa = a.nab / a.nsb, nsc = a.ncd / a.nsd;
+        for (int e = tid; e < nsa * nsc; e += nthr) {
+            const double v = sK[e];
+            if (v != 0.0) atomicAdd(a.K + (size_t)(k_ao_a + e / nsc) * a.nbf + k_ao_c + e % nsc, v);
+        }
+    }
 }
 
 // Splits the nrb_ab eight-row blocks of a quartet into work items of at most 11 blocks (one consumer warp
@@ -436,10 +517,10 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
     // ring depth: whatever shared memory is left after R, at least 2 stages, at most MAX_STAGES
     int nst = 2;
     for (int s = MAX_STAGES; s >= 2; --s)
-        if (SmemLayout(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, s).total <= budget) { nst = s; break; }
+        if (SmemLayout(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, s, a.digest).total <= budget) { nst = s; break; }
     if (nst > a.ncb_q) nst = a.ncb_q < 2 ? 2 : a.ncb_q;
     a.nst = nst;
-    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, nst);
+    const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, nst, a.digest);
     if (lay.total > budget) {
         if (MINB > 1) return launch_one<NT_CD, NQT, MAXW, EXACT, 1>(ctx, a, st);
         ctx->err = "md4_compute: shared memory needed exceeds the device limit";
@@ -488,8 +569,13 @@ void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows) {
 }
 
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
-                      cudaStream_t st) {
+                      cudaStream_t st, const DigestArgs* dg) {
     EriArgs a;
+    a.digest = dg ? 1 : 0;
+    a.nbf = dg ? dg->nbf : 0;
+    a.nsb = n_solid(bra.lj); a.nsd = n_solid(ket.lj);
+    a.aob = bra.ao; a.aok = ket.ao;
+    a.D = dg ? dg->D : nullptr; a.J = dg ? dg->J : nullptr; a.K = dg ? dg->K : nullptr;
     a.Hb = bra.Hb; a.sb = bra.scal; a.pmb = bra.pairmax; a.hsb = bra.hstrideb;
     a.Hk = ket.Hk; a.sk = ket.scal; a.pmk = ket.pairmax; a.hsk = ket.hstridek;
     a.Kb = bra.Ki * bra.Kj; a.Kk = ket.Ki * ket.Kj; a.nbra = bra.npair; a.nket = ket.npair;

@@ -94,6 +94,16 @@ struct PairListDev {
     double* scal;        // [npair*Ki*Kj * 8]: zeta_p, Px, Py, Pz, lnK - pairmax, 0, 0, 0
     double* pairmax;     // [npair] max over primitives of ln K_ab
     int* ij;             // [npair*2]
+    int* ao;             // [npair*2] first AO (solid-harmonic function) of shells i and j in the shell set the list was built from
+    int nbf;             // number of AOs of that shell set
+};
+
+// direct digestion (md4_compute_jk): AO-basis density in, Coulomb- / exchange-type matrices out (either may be null)
+struct DigestArgs {
+    int nbf;
+    const double* D;
+    double* J;
+    double* K;
 };
 
 // Interaction kernel (md4_device.cuh kernel_seed): G_m = ka F_m(T) + kb s^(2m+1) F_m(s^2 T), s^2 = omega2/(omega2 + rho)
@@ -140,7 +150,7 @@ struct md4_ctx {
     int* d_off = nullptr;
     double* d_exp = nullptr;
     double* d_coef = nullptr;
-    std::vector<int> h_l, h_off;
+    std::vector<int> h_l, h_off, h_ao;   // h_ao: first AO of every shell, h_ao[nshell] = number of AOs
     std::set<md4_pairs*> lists;
     // released pair-list blocks kept for the next md4_build_pairs (workspaces grow only, S:8(b)): a batch loop that
     // builds and frees pair lists every step then never reaches cudaMalloc/cudaFree (both synchronise the device)
@@ -175,7 +185,7 @@ namespace md4 {
 cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t st);
 // md4_eri.cu
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
-                      cudaStream_t st);
+                      cudaStream_t st, const DigestArgs* dg = nullptr);
 void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows);   // the work-item split of md4_compute (host logic)
 cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, double* d_out);
 cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out);

@@ -21,7 +21,7 @@ STATUS_NAMES = ["MD4_OK", "MD4_EINVAL", "MD4_EUNSUPPORTED", "MD4_ESTATE", "MD4_E
 #: every symbol include/md4.h declares (tests check the library exports exactly these)
 SYMBOLS = [
     "md4_create", "md4_destroy", "md4_last_error", "md4_set_shells", "md4_build_pairs", "md4_free_pairs",
-    "md4_stream_wait_pairs", "md4_set_kernel",
+    "md4_stream_wait_pairs", "md4_set_kernel", "md4_num_ao", "md4_compute_jk", "md4_compute_jk_host",
     "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host",
     "md4_launch_count", "md4_flops_per_quartet", "md4_debug_boys", "md4_debug_solid_coeff",
     "md4_debug_hermite_r", "md4_debug_pair_h", "md4_debug_work_items",
@@ -72,6 +72,12 @@ def load():
     lib.md4_compute.restype = ctypes.c_int
     lib.md4_compute_host.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, vp]
     lib.md4_compute_host.restype = ctypes.c_int
+    lib.md4_num_ao.argtypes = [vp, ip]
+    lib.md4_num_ao.restype = ctypes.c_int
+    lib.md4_compute_jk.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.md4_compute_jk.restype = ctypes.c_int
+    lib.md4_compute_jk_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.md4_compute_jk_host.restype = ctypes.c_int
     lib.md4_launch_count.argtypes = [vp]
     lib.md4_launch_count.restype = ctypes.c_longlong
     lib.md4_flops_per_quartet.argtypes = [vp, vp]
@@ -220,6 +226,39 @@ class Engine:
         self._check(load().md4_compute_host(self.handle, bra.handle, ket.handle, ctypes.c_void_p(out.ctypes.data),
                                             out.size, ctypes.c_void_p(stream)))
         return out.reshape(-1)[:n].reshape(self.output_shape(bra, ket))
+
+    def num_ao(self) -> int:
+        n = ctypes.c_int()
+        self._check(load().md4_num_ao(self.handle, ctypes.byref(n)))
+        return int(n.value)
+
+    def compute_jk(self, bra: PairList, ket: PairList, D, J=None, K=None, stream=None):
+        """Enqueue md4_compute_jk: J[a,b] += sum_cd (ab|cd) D[c,d], K[a,c] += sum_bd (ab|cd) D[b,d] on [nbf, nbf] float64 CUDA
+        tensors (J / K are accumulated into; pass None to skip one)."""
+        import torch
+
+        def ptr(t):
+            if t is None:
+                return ctypes.c_void_p(0)
+            if t.dtype != torch.float64 or not t.is_cuda or not t.is_contiguous():
+                raise ValueError("D, J, K must be contiguous float64 CUDA tensors")
+            return ctypes.c_void_p(t.data_ptr())
+
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        self._check(load().md4_compute_jk(self.handle, bra.handle, ket.handle, ptr(D), ptr(J), ptr(K), ctypes.c_void_p(stream)))
+
+    def compute_jk_host(self, bra: PairList, ket: PairList, D: np.ndarray, J: np.ndarray | None = None,
+                        K: np.ndarray | None = None, stream: int = 0):
+        """md4_compute_jk_host on float64 numpy matrices (J / K accumulated in place)."""
+        def ptr(x):
+            if x is None:
+                return ctypes.c_void_p(0)
+            if x.dtype != np.float64 or not x.flags.c_contiguous:
+                raise ValueError("D, J, K must be C-contiguous float64 arrays")
+            return ctypes.c_void_p(x.ctypes.data)
+
+        self._check(load().md4_compute_jk_host(self.handle, bra.handle, ket.handle, ptr(D), ptr(J), ptr(K), ctypes.c_void_p(stream)))
 
     def launch_count(self) -> int:
         return int(load().md4_launch_count(self.handle))

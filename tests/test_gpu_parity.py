@@ -503,3 +503,78 @@ def test_attenuated_kernels_add_up_on_the_gpu(eng, coulomb_after):
     with pytest.raises(Exception):
         eng.set_kernel("erf", -1.0)
     bra.free(); ket.free()
+
+
+# ------------------------------------------------------------- direct digestion (S:8(f) item 2)
+def _jk_check(eng, wl, seed, both=True):
+    import torch
+
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    nbf = eng.num_ao()
+    rng = np.random.Generator(np.random.PCG64(seed))
+    D = rng.uniform(-1.0, 1.0, (nbf, nbf))
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    dD = torch.from_numpy(D).cuda()
+    J = torch.zeros(nbf, nbf, dtype=torch.float64, device="cuda")
+    K = torch.zeros_like(J)
+    eng.compute_jk(bra, ket, dD, J, K if both else None)
+    torch.cuda.synchronize()
+    Jr, Kr = oracle.digest_jk(_oshells(s), wl.bra_ij, wl.ket_ij, D)
+    assert oracle.ao_offsets(_oshells(s))[-1] == nbf
+    # J and K are sums over quartets of very different size: the bar is 1e-10 of the largest element of the matrix
+    assert np.abs(J.cpu().numpy() - Jr.astype(np.float64)).max() <= TOL * np.abs(Jr).max()
+    if both:
+        assert np.abs(K.cpu().numpy() - Kr.astype(np.float64)).max() <= TOL * np.abs(Kr).max()
+    # the host form accumulates into what it is given
+    J0 = rng.uniform(-1.0, 1.0, (nbf, nbf)) * float(np.abs(Jr).max())
+    Jh, Kh = J0.copy(), np.zeros((nbf, nbf))
+    eng.compute_jk_host(bra, ket, D, Jh, Kh)
+    assert np.abs(Jh - J0 - Jr.astype(np.float64)).max() <= 10 * TOL * np.abs(Jr).max()
+    assert np.abs(Kh - Kr.astype(np.float64)).max() <= TOL * np.abs(Kr).max()
+    bra.free(); ket.free()
+
+
+@pytest.mark.parametrize("lclass,kclass", [((0, 0, 0, 0), (1, 1, 1, 1)), ((2, 1, 1, 2), (1, 2, 1, 1)), ((4, 4, 4, 4), (1, 1, 1, 1)),
+                                           ((5, 4, 6, 4), (1, 1, 1, 1)), ((6, 5, 4, 4), (1, 1, 1, 1)), ((6, 6, 6, 6), (1, 1, 1, 1)),
+                                           ((6, 6, 6, 5), (2, 1, 1, 2))])
+def test_digest_jk_small_classes(eng, lclass, kclass):
+    """md4_compute_jk against the oracle leg (binary128 integrals, long-double contraction) on ragged 5 x 4 batches:
+    every element of J and K."""
+    wl = inputs.small_workload(lclass, kclass, nbra=5, nket=4, seed=61)
+    _jk_check(eng, wl, 62)
+
+
+def test_digest_jk_config1(eng):
+    """cfg 1 (gg|gg): all 256 quartets digested; 16 shells -> 144 AOs."""
+    _jk_check(eng, inputs.config1(), 63)
+
+
+def test_digest_jk_equals_contraction_of_stored_integrals(eng):
+    """Full-size launch (cfg2, 4096 (hh|hh) quartets, CTAs walk through ~55 items each): J and K from the digesting
+    epilogue against the same contraction done with torch on the integrals md4_compute stores (independent of the oracle,
+    covers every quartet of the launch)."""
+    import torch
+
+    wl = inputs.config2()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    nbf = eng.num_ao()
+    off = np.concatenate([[0], np.cumsum(2 * s.l + 1)])
+    g = torch.Generator(device="cuda").manual_seed(7)
+    D = torch.rand(nbf, nbf, dtype=torch.float64, device="cuda", generator=g) - 0.5
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    eri = eng.compute(bra, ket)
+    J = torch.zeros(nbf, nbf, dtype=torch.float64, device="cuda"); K = torch.zeros_like(J)
+    eng.compute_jk(bra, ket, D, J, K)
+    torch.cuda.synchronize()
+    Jr = torch.zeros_like(J); Kr = torch.zeros_like(K)
+    n = 11
+    for i, (a, b) in enumerate(wl.bra_ij):
+        for j, (c, d) in enumerate(wl.ket_ij):
+            blk = eri[i, j]
+            Jr[off[a]:off[a] + n, off[b]:off[b] + n] += torch.einsum("abcd,cd->ab", blk, D[off[c]:off[c] + n, off[d]:off[d] + n])
+            Kr[off[a]:off[a] + n, off[c]:off[c] + n] += torch.einsum("abcd,bd->ac", blk, D[off[b]:off[b] + n, off[d]:off[d] + n])
+    assert ((J - Jr).abs().max() / Jr.abs().max()).item() <= 1e-12
+    assert ((K - Kr).abs().max() / Kr.abs().max()).item() <= 1e-12
+    bra.free(); ket.free()
