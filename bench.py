@@ -373,6 +373,34 @@ def run_gpu(args):
     e2e_s = reduce_max(time.perf_counter() - w0, world, f"cuda:{local}")
     e2e_value = whole_job_rate(world, nq, 1e3 * e2e_s / args.steps)
 
+    # ---- end to end with direct digestion: the same K steps, but the integrals are contracted with
+    # an AO density on the device (md4_compute_jk_host: J and K out) instead of being shipped to the host
+    dg_rng = np.random.Generator(np.random.PCG64(99))
+    dg_bufs = []
+    for wl in wls:
+        nbf = int((2 * wl.shells.l + 1).sum())
+        dg_bufs.append((dg_rng.uniform(-1.0, 1.0, (nbf, nbf)), np.zeros((nbf, nbf)), np.zeros((nbf, nbf))))
+    dg_h2d = int(sum(w.shells.centers.nbytes + w.shells.l.nbytes + w.shells.prim_offset.nbytes + w.shells.exponents.nbytes +
+                     w.shells.coefficients.nbytes + w.bra_ij.nbytes + w.ket_ij.nbytes + 3 * b[0].nbytes for w, b in zip(wls, dg_bufs)))
+    dg_d2h = int(sum(2 * b[0].nbytes for b in dg_bufs))
+
+    def digest_step():
+        for wl, (D, J, K) in zip(wls, dg_bufs):
+            upload(wl)
+            bra = eng.build_pairs(wl.bra_ij)
+            ket = eng.build_pairs(wl.ket_ij)
+            eng.compute_jk_host(bra, ket, D, J, K, stream=stream.cuda_stream)
+            bra.free(); ket.free()
+
+    digest_step()
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(args.steps):
+        digest_step()
+    barrier()
+    dg_s = reduce_max(time.perf_counter() - w0, world, f"cuda:{local}")
+    dg_value = whole_job_rate(world, nq, 1e3 * dg_s / args.steps)
+
     if rank == 0:
         peak, peak_how = fp64_peak_tflops()
         traffic, traffic_src = ncu_traffic(args.workload)
@@ -391,6 +419,9 @@ def run_gpu(args):
                          "algorithmic_bytes": int(sum(out_doubles) * 8),
                          "peak_source": peak_how, "kernel_ms": k_ms},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "e2e_digest": {"value": dg_value, "unit": UNIT, "h2d_bytes_per_step": dg_h2d, "d2h_bytes_per_step": dg_d2h,
+                           "what": "md4_set_shells + md4_build_pairs x2 + md4_compute_jk_host: (ab|cd) contracted with an AO density "
+                                   "in the kernel epilogue (J and K to the host) instead of 8 Nab Ncd bytes per quartet"},
             "gpu_launches": int(n_launch), "clocks": clocks,
         }
         if multi:

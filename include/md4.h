@@ -40,7 +40,9 @@
 extern "C" {
 #endif
 
-#define MD4_LMAX 6 /* highest per-shell angular momentum accepted (i functions) */
+#define MD4_LMAX 7 /* highest per-shell angular momentum accepted (k functions; "can be extended") */
+#define MD4_LSUM_MAX 24 /* md4_compute needs l_a + l_b + l_c + l_d <= 24 (Hermite tensor R in shared memory), l_c + l_d <= 12
+                           and (2l_c+1)(2l_d+1) <= 176: every class of l <= 6 shells, and l = 7 shells with lighter partners */
 
 typedef struct md4_ctx md4_ctx;     /* opaque engine, one per CUDA device                     */
 typedef struct md4_pairs md4_pairs; /* opaque shell-pair list (device resident), owned by ctx  */
@@ -48,7 +50,7 @@ typedef struct md4_pairs md4_pairs; /* opaque shell-pair list (device resident),
 typedef enum {
     MD4_OK = 0,
     MD4_EINVAL = 1,       /* bad argument: null pointer, index out of range, class mix, zeta <= 0 */
-    MD4_EUNSUPPORTED = 2, /* l > MD4_LMAX                                                          */
+    MD4_EUNSUPPORTED = 2, /* l > MD4_LMAX, or a quartet class beyond MD4_LSUM_MAX                          */
     MD4_ESTATE = 3,       /* call order: pairs before shells, pairs of another context             */
     MD4_ENOMEM = 4,       /* host or device allocation failed                                      */
     MD4_ECUDA = 5         /* CUDA runtime error; text in md4_last_error                            */
@@ -70,7 +72,7 @@ const char* md4_last_error(const md4_ctx* ctx);
  * exponents, contraction coefficients.  Replaces any previous shell set; existing pair lists stay
  * valid (they hold their own data).
  *   centers_xyz   HOST [nshell*3]  bohr
- *   l             HOST [nshell]    0..MD4_LMAX
+ *   l             HOST [nshell]    0..MD4_LMAX (7; see MD4_LSUM_MAX for the classes md4_compute accepts)
  *   prim_offset   HOST [nshell+1]  CSR offsets into exponents/coefficients, prim_offset[0] = 0, increasing
  *   exponents     HOST [nprim]     > 0, finite
  *   coefficients  HOST [nprim]     finite, applied verbatim
@@ -174,7 +176,7 @@ double md4_flops_per_quartet(const md4_pairs* bra, const md4_pairs* ket);
 /* ---- stage-level access for the parity tests (S:4 test layer 3) --------------------------------- */
 
 /* How md4_compute splits the (2li+1)(2lj+1) rows of a bra class into work items of 8-row blocks, one consumer warp
- * per block (host logic only, no device needed): out7 HOST [7] = number of items per quartet (1 or 2), first row
+ * per block (host logic only, no device needed): out7 HOST [7] = number of items per quartet (1 to 3), first row
  * block of item 0..2, row blocks of item 0..2.  The FP64 tensor pipe of sm_100a is per SM sub-partition, so an item
  * of n blocks costs ceil(n/4) block-times; the split minimises their sum. */
 md4_status md4_debug_work_items(int li, int lj, int* out7);

@@ -497,14 +497,19 @@ void plan_items(EriArgs& a) {
     const int n = a.nrb_ab;
     for (int t = 0; t < 3; ++t) { a.row0[t] = 0; a.nrows[t] = 0; }
     if (n <= 11) { a.ncta_per_q = 1; a.nrows[0] = n; a.wpc = n; return; }
-    int best = 1 << 30, b1 = 0;
-    for (int n1 = (n + 1) / 2; n1 <= 11; ++n1) {
-        const int n2 = n - n1;
-        const int cost = ((n1 + 3) / 4 + (n2 + 3) / 4) * 16 + n1;
-        if (cost < best) { best = cost; b1 = n1; }
-    }
-    a.ncta_per_q = 2;
-    a.nrows[0] = b1; a.row0[1] = b1; a.nrows[1] = n - b1;
+    // two items if they can hold the rows (n <= 22), else three (l = 7 bras: up to 29 row blocks)
+    const int k = n <= 22 ? 2 : 3;
+    int best = 1 << 30, b1 = 0, b2 = 0;
+    for (int n1 = 1; n1 <= 11; ++n1)
+        for (int n2 = (k == 2 ? n - n1 : 1); n2 <= (k == 2 ? n - n1 : 11); ++n2) {
+            const int n3 = n - n1 - n2;
+            if (n2 < 1 || n2 > n1 || n3 < 0 || n3 > n2 || n3 > 11 || (k == 3 && n3 < 1)) continue;
+            const int cost = ((n1 + 3) / 4 + (n2 + 3) / 4 + (n3 + 3) / 4) * 16 + n1;
+            if (cost < best) { best = cost; b1 = n1; b2 = n2; }
+        }
+    a.ncta_per_q = k;
+    a.nrows[0] = b1; a.row0[1] = b1; a.nrows[1] = b2;
+    if (k == 3) { a.row0[2] = b1 + b2; a.nrows[2] = n - b1 - b2; }
     a.wpc = b1;
 }
 
@@ -582,9 +587,13 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     a.nab = bra.nab; a.ncd = ket.nab; a.nrb_ab = bra.nrb; a.nrb_cd = ket.nrb;
     a.ncb_p = bra.ncbb; a.ncb_q = ket.ncbk;
     a.L = bra.lsum + ket.lsum;
+    if (a.L > LTOT || ket.lsum > LKET_MAX || ket.nrb > 22) {
+        ctx->err = "md4_compute: class beyond MD4_LSUM_MAX (needs l_a+l_b+l_c+l_d <= 24, l_c+l_d <= 12, (2l_c+1)(2l_d+1) <= 176)";
+        return MD4_EUNSUPPORTED;
+    }
     plan_items(a);
     a.nquartets = (long long)a.nbra * a.nket;
-    a.qmajor = (a.ncta_per_q == 2 && a.nrows[0] != a.nrows[1]) ? 1 : 0;
+    a.qmajor = (a.ncta_per_q >= 2 && a.nrows[0] != a.nrows[a.ncta_per_q - 1]) ? 1 : 0;
     // strip height: the H matrices of a strip's bra pairs (K_bra matrices each) should stay L2-resident next to the kets
     // in flight: <= 16 MB per strip.  Measured on cfg3 / cfg5 (ii|ii) K=3: flat order 58.0 / 923 ms, 32-pair strips
     // 57.8 / 962 ms (a contracted strip of 32 is 185 MB), this rule 57.8 / 923 ms.
@@ -612,6 +621,7 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     if (nt <= 4) return launch_small<4>(ctx, a, st);
     if (nt <= 7) return launch_small<7>(ctx, a, st);
     if (nt <= 12) return launch_w<12, false>(ctx, a, st);
+    if (nt <= 22) return launch_w<22, false>(ctx, a, st);   // kets with an l = 7 shell: 15 x 9 = 135 (17 blocks), 15 x 11 = 165 (21)
     ctx->err = "md4_compute: ket class too large";
     return MD4_EUNSUPPORTED;
 }

@@ -13,7 +13,10 @@
 namespace md4 {
 
 constexpr int LMAX = MD4_LMAX;          // per shell
-constexpr int LTOT = 4 * LMAX;          // highest Hermite order L = la+lb+lc+ld
+constexpr int LTOT = MD4_LSUM_MAX;      // highest Hermite order L = la+lb+lc+ld the fused kernel takes: R in the additive
+                                        // layout (121 kB at L = 24) must fit shared memory next to the ring; l = 7 shells are
+                                        // accepted in classes up to this L (S:8(f) item 4)
+constexpr int LKET_MAX = 12;            // highest l_c + l_d: 57 q~ column blocks (TACC_QBLOCKS), <= 22 accumulator tiles per lane
 constexpr int NR_MAX = (LTOT + 1) * (LTOT + 2) * (LTOT + 3) / 6;  // 2925
 
 // Boys table: nodes T_j = j / BOYS_INV_DELTA, j = 0..BOYS_NODES-1, values F_m(T_j) for m = 0..BOYS_STRIDE-1.

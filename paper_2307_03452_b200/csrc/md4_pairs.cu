@@ -9,11 +9,11 @@
 namespace md4 {
 
 namespace {
-constexpr int NA1 = LMAX + 1;          // a_i = 0..6
-constexpr int NT1 = 2 * LMAX + 1;      // t = 0..12
-constexpr int ESZ = NA1 * NA1 * NT1;   // 637 per axis
-constexpr int NCMAX = (LMAX + 1) * (LMAX + 2) / 2;  // 28
-constexpr int NSMAX = 2 * LMAX + 1;    // 13
+constexpr int NA1 = LMAX + 1;          // a_i = 0..LMAX
+constexpr int NT1 = 2 * LMAX + 1;      // t = 0..2 LMAX
+constexpr int ESZ = NA1 * NA1 * NT1;   // 960 per axis at LMAX = 7 (637 at 6)
+constexpr int NCMAX = (LMAX + 1) * (LMAX + 2) / 2;  // 36
+constexpr int NSMAX = 2 * LMAX + 1;    // 15
 constexpr int PAIR_THREADS = 256;
 constexpr int PAIR_SPLIT = 8;          // CTAs per primitive pair (each takes a range of Hermite column blocks)
 

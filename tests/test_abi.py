@@ -93,17 +93,19 @@ def test_product_never_imports_oracle():
 def test_work_item_split_follows_the_sub_partition_rule(lib):
     """Host logic of md4_compute (no GPU): rows of a bra class -> work items of <= 11 eight-row blocks.  An item of n
     blocks costs ceil(n/4) block-times (FP64 tensor pipe per SM sub-partition, profiles/r1_fp64_peak.txt): the split
-    must cover every row block exactly once and reach the minimum ceil(nrb/4) whenever two items can."""
+    must cover every row block exactly once and reach the minimum ceil(nrb/4); bras with an l = 7 shell (up to 29 row
+    blocks) take three items."""
     from paper_2307_03452_b200 import md4
 
-    expect = {(6, 6): [11, 11], (6, 5): [10, 8], (5, 5): [8, 8], (6, 4): [8, 7], (5, 4): [7, 6], (4, 4): [11], (2, 2): [4]}
-    for li in range(7):
+    expect = {(6, 6): [11, 11], (6, 5): [10, 8], (5, 5): [8, 8], (6, 4): [8, 7], (5, 4): [7, 6], (4, 4): [11], (2, 2): [4],
+              (7, 7): [11, 10, 8], (7, 6): [9, 8, 8], (7, 4): [9, 8]}
+    for li in range(8):
         for lj in range(li + 1):
             nrb = ((2 * li + 1) * (2 * lj + 1) + 7) // 8
             n, row0, nrows = md4.work_items(li, lj)
             assert sum(nrows) == nrb and all(1 <= r <= 11 for r in nrows)
             assert row0 == [sum(nrows[:i]) for i in range(n)]
-            assert n == (1 if nrb <= 11 else 2)
+            assert n == (1 if nrb <= 11 else 2 if nrb <= 22 else 3)
             assert sum((r + 3) // 4 for r in nrows) == (nrb + 3) // 4
             if (li, lj) in expect:
                 assert nrows == expect[(li, lj)], (li, lj, nrows)

@@ -94,7 +94,7 @@ def test_boys_stage(eng):
 
 def test_solid_coeff_stage(eng):
     """P:109-113 Eq.16 coefficients: the library's recurrence-generated table vs the oracle's closed-sum table."""
-    for l in range(7):
+    for l in range(8):
         got = eng.debug_solid_coeff(l)
         ref = oracle.solid_coeff(l).astype(np.float64)
         assert got.shape == ref.shape
@@ -118,7 +118,8 @@ def test_hermite_r_stage(eng, L, zp, zq, P, Q):
         assert np.abs(g - r).max() <= _r_stage_tol(n) * np.abs(r).max(), (n, np.abs(g - r).max() / np.abs(r).max())
 
 
-@pytest.mark.parametrize("lclass,kclass", [((2, 1, 0, 0), (1, 1, 1, 1)), ((4, 3, 0, 0), (2, 1, 1, 1)), ((6, 6, 0, 0), (1, 1, 1, 1))])
+@pytest.mark.parametrize("lclass,kclass", [((2, 1, 0, 0), (1, 1, 1, 1)), ((4, 3, 0, 0), (2, 1, 1, 1)), ((6, 6, 0, 0), (1, 1, 1, 1)),
+                                           ((7, 5, 0, 0), (1, 1, 1, 1))])
 def test_pair_h_stage(eng, lclass, kclass):
     """S:8(a) a1.  H, zeta_p, R_p, ln K_ab from the pair kernel vs a 40-digit E recursion (Eq.4-5) contracted
     with the oracle's solid-harmonic tables (Eq.16)."""
@@ -315,7 +316,7 @@ def test_empty_lists_and_errors(eng):
         eng.build_pairs(np.array([[0, 999]], dtype=np.int32))
     assert ei.value.status == md4.MD4_EINVAL
     with pytest.raises(md4.Md4Error) as ei:
-        eng.set_shells([[0, 0, 0]], [7], [0, 1], [1.0], [1.0])
+        eng.set_shells([[0, 0, 0]], [8], [0, 1], [1.0], [1.0])
     assert ei.value.status == md4.MD4_EUNSUPPORTED
     with pytest.raises(md4.Md4Error) as ei:
         eng.set_shells([[0, 0, 0]], [1], [0, 1], [-1.0], [1.0])
@@ -578,3 +579,40 @@ def test_digest_jk_equals_contraction_of_stored_integrals(eng):
     assert ((J - Jr).abs().max() / Jr.abs().max()).item() <= 1e-12
     assert ((K - Kr).abs().max() / Kr.abs().max()).item() <= 1e-12
     bra.free(); ket.free()
+
+
+# ------------------------------------------------------------------------ l = 7 shells (S:8(f) item 4)
+K_CLASSES = [((7, 0, 0, 0), (1, 1, 1, 1)), ((7, 7, 2, 2), (1, 1, 1, 1)), ((7, 4, 4, 4), (1, 2, 1, 1)), ((7, 7, 5, 5), (1, 1, 1, 1)),
+             ((6, 6, 7, 3), (1, 1, 1, 1)), ((4, 4, 7, 5), (1, 1, 1, 1)), ((7, 6, 6, 5), (1, 1, 1, 1)), ((3, 7, 7, 1), (2, 1, 1, 1))]
+
+
+@pytest.mark.parametrize("lclass,kclass", K_CLASSES)
+def test_k_shell_classes(eng, lclass, kclass):
+    """l = 7 (k) shells ("can be extended"): bras of up to 15 x 15 = 225 functions (29 row blocks, three work items),
+    kets with a k shell up to (kh| (165 functions), total L up to 24 -- every element against the binary128 oracle."""
+    for nbra, nket, seed in ((3, 2, 71), (1, 4, 72)):
+        wl = inputs.small_workload(lclass, kclass, nbra=nbra, nket=nket, seed=seed)
+        g, r = _run(eng, wl)
+        errs, below = _quartet_errors(g, r)
+        assert below == 0
+        assert errs.max() <= TOL, (lclass, kclass, errs.max())
+
+
+def test_k_shell_class_limits(eng):
+    """Classes beyond MD4_LSUM_MAX are refused with MD4_EUNSUPPORTED and nothing is enqueued: (kk|kk) (L = 28),
+    (ii|kk) (ket of 225 functions), (kk|ii) (L = 26)."""
+    import torch
+    from paper_2307_03452_b200 import md4
+
+    for lclass in ((7, 7, 7, 7), (6, 6, 7, 7), (7, 7, 6, 6)):
+        wl = inputs.small_workload(lclass, nbra=1, nket=1, seed=73)
+        s = wl.shells
+        eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+        bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+        n0 = eng.launch_count()
+        with pytest.raises(md4.Md4Error) as ei:
+            eng.compute(bra, ket)
+        assert ei.value.status == md4.MD4_EUNSUPPORTED and "MD4_LSUM_MAX" in eng.last_error()
+        assert eng.launch_count() == n0
+        bra.free(); ket.free()
+    torch.cuda.synchronize()
