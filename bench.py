@@ -376,10 +376,14 @@ def run_gpu(args):
     # ---- end to end with direct digestion: the same K steps, but the integrals are contracted with
     # an AO density on the device (md4_compute_jk_host: J and K out) instead of being shipped to the host
     dg_rng = np.random.Generator(np.random.PCG64(99))
-    dg_bufs = []
+    dg_bufs, dg_keep = [], []
     for wl in wls:
         nbf = int((2 * wl.shells.l + 1).sum())
-        dg_bufs.append((dg_rng.uniform(-1.0, 1.0, (nbf, nbf)), np.zeros((nbf, nbf)), np.zeros((nbf, nbf))))
+        pin = [torch.empty(nbf, nbf, dtype=torch.float64, pin_memory=True) for _ in range(3)]   # D, J, K in pinned host memory
+        dg_keep.append(pin)
+        D, J, K = (t.numpy() for t in pin)
+        D[:] = dg_rng.uniform(-1.0, 1.0, (nbf, nbf)); J[:] = 0.0; K[:] = 0.0
+        dg_bufs.append((D, J, K))
     dg_h2d = int(sum(w.shells.centers.nbytes + w.shells.l.nbytes + w.shells.prim_offset.nbytes + w.shells.exponents.nbytes +
                      w.shells.coefficients.nbytes + w.bra_ij.nbytes + w.ket_ij.nbytes + 3 * b[0].nbytes for w, b in zip(wls, dg_bufs)))
     dg_d2h = int(sum(2 * b[0].nbytes for b in dg_bufs))

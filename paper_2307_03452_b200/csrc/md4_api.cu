@@ -86,10 +86,19 @@ cudaError_t pool_alloc(md4_ctx* c, size_t bytes, PoolBlock* out) {
     return e;
 }
 
-// c == nullptr: the context is going away (everything has been synchronised), free for real
+// c == nullptr: the context is going away (everything has been synchronised), free for real.  A block that would push
+// the pool over its cap evicts the smallest idle blocks first (a sweep over many classes otherwise fills the pool with
+// small blocks and then frees -- and re-allocates -- the big ones on every step).
 void pool_free(md4_ctx* c, PoolBlock blk) {
     if (!blk.p) { if (blk.ev) cudaEventDestroy(blk.ev); return; }
-    if (c && blk.bytes >= POOL_MIN_BYTES && c->pool_bytes + blk.bytes <= c->pool_max_bytes) {
+    if (c && blk.bytes >= POOL_MIN_BYTES && blk.bytes <= c->pool_max_bytes) {
+        while (c->pool_bytes + blk.bytes > c->pool_max_bytes && !c->pool.empty()) {
+            auto it = c->pool.begin();
+            if (it->second.ev) { cudaEventSynchronize(it->second.ev); cudaEventDestroy(it->second.ev); }
+            cudaFree(it->second.p);
+            c->pool_bytes -= it->second.bytes;
+            c->pool.erase(it);
+        }
         c->pool.emplace(blk.bytes, blk);
         c->pool_bytes += blk.bytes;
     } else {

@@ -9,10 +9,6 @@
 namespace md4 {
 
 namespace {
-constexpr int NA1 = LMAX + 1;          // a_i = 0..LMAX
-constexpr int NT1 = 2 * LMAX + 1;      // t = 0..2 LMAX
-constexpr int ESZ = NA1 * NA1 * NT1;   // 960 per axis at LMAX = 7 (637 at 6)
-constexpr int NCMAX = (LMAX + 1) * (LMAX + 2) / 2;  // 36
 constexpr int NSMAX = 2 * LMAX + 1;    // 15
 constexpr int PAIR_THREADS = 256;
 constexpr int PAIR_SPLIT = 8;          // CTAs per primitive pair (each takes a range of Hermite column blocks)
@@ -68,17 +64,42 @@ struct PairKernelArgs {
     size_t hstrideb, hstridek;
 };
 
-struct PairSmem {
-    dd E[3][ESZ];
-    dd Ca[NSMAX * NCMAX];
-    dd Cb[NSMAX * NCMAX];
-    dd Y[NCMAX * NSMAX * 8];
-    unsigned char ca[NCMAX][2], cb[NCMAX][2];
+// Shared memory of one CTA, sized for the class of the list (li, lj), not for MD4_LMAX: an (ii) list takes 87 kB (two
+// CTAs per SM), a (gg) list 33 kB, a (kk) list 132 kB.  1-D tables E[axis][(ai * na1 + bi) * nt1 + t] with na1 =
+// max(li, lj) + 1 and nt1 = li + lj + 1.
+struct PairSmemLayout {
+    int na1, nt1, esz;
+    size_t oE, oCa, oCb, oY, oca, ocb, total;
+    __host__ __device__ PairSmemLayout(int li, int lj) {
+        na1 = (li > lj ? li : lj) + 1;
+        nt1 = li + lj + 1;
+        esz = na1 * na1 * nt1;
+        const int nca = n_cart(li), ncb = n_cart(lj), nsa = 2 * li + 1, nsb = 2 * lj + 1;
+        size_t o = 0;
+        oE = o; o += (size_t)3 * esz * sizeof(dd);
+        oCa = o; o += (size_t)nsa * nca * sizeof(dd);
+        oCb = o; o += (size_t)nsb * ncb * sizeof(dd);
+        oY = o; o += (size_t)nca * nsb * 8 * sizeof(dd);
+        oca = o; o += (size_t)nca * 2;
+        ocb = o; o += (size_t)ncb * 2;
+        total = (o + 15) / 16 * 16;
+    }
 };
 
 __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) {
     extern __shared__ __align__(16) unsigned char pair_smem_raw[];
-    PairSmem& sm = *reinterpret_cast<PairSmem*>(pair_smem_raw);
+    const PairSmemLayout lay(a.li, a.lj);
+    const int NA1 = lay.na1, NT1 = lay.nt1, ESZ = lay.esz;
+    struct {
+        dd* E[3]; dd* Ca; dd* Cb; dd* Y;
+        unsigned char (*ca)[2]; unsigned char (*cb)[2];
+    } sm;
+    for (int i = 0; i < 3; ++i) sm.E[i] = reinterpret_cast<dd*>(pair_smem_raw + lay.oE) + (size_t)i * ESZ;
+    sm.Ca = reinterpret_cast<dd*>(pair_smem_raw + lay.oCa);
+    sm.Cb = reinterpret_cast<dd*>(pair_smem_raw + lay.oCb);
+    sm.Y = reinterpret_cast<dd*>(pair_smem_raw + lay.oY);
+    sm.ca = reinterpret_cast<unsigned char (*)[2]>(pair_smem_raw + lay.oca);
+    sm.cb = reinterpret_cast<unsigned char (*)[2]>(pair_smem_raw + lay.ocb);
 
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int split = blockIdx.x % PAIR_SPLIT;
@@ -104,7 +125,7 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
         XPB[i] = -(za / zp) * d;
         ab2 += d * d;
     }
-    for (int i = tid; i < 3 * ESZ; i += nthr) (&sm.E[0][0])[i] = make_double2(0.0, 0.0);
+    for (int i = tid; i < 3 * ESZ; i += nthr) sm.E[0][i] = make_double2(0.0, 0.0);   // the three tables are contiguous
     for (int i = tid; i < nsa * nca; i += nthr) sm.Ca[i] = make_double2(a.Ca[i], a.CaLo[i]);
     for (int i = tid; i < nsb * ncbt; i += nthr) sm.Cb[i] = make_double2(a.Cb[i], a.CbLo[i]);
     if (tid == 0) {
@@ -126,7 +147,7 @@ __global__ void __launch_bounds__(PAIR_THREADS) pair_h_kernel(PairKernelArgs a) 
     // lane t does Hermite order t; one step of the recurrence per __syncwarp.
     const int warp = tid >> 5, lane = tid & 31;
     if (warp < 3) {
-        dd* E = sm.E[warp];
+        dd* E = sm.E[0] + (size_t)warp * ESZ;
         const double xpa = XPA[warp], xpb = XPB[warp], h = 0.5 / zp;
         if (lane == 0) E[0] = make_double2(1.0, 0.0);
         __syncwarp();
@@ -241,10 +262,10 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
     const size_t nblk = nprim * PAIR_SPLIT;
     if (nblk > 2147483647ull) return cudaErrorInvalidValue;
     if (ctx->configured.insert(reinterpret_cast<const void*>(pair_h_kernel)).second) {
-        e = cudaFuncSetAttribute(pair_h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PairSmem));
+        e = cudaFuncSetAttribute(pair_h_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PairSmemLayout(LMAX, LMAX).total);
         if (e != cudaSuccess) { ctx->configured.erase(reinterpret_cast<const void*>(pair_h_kernel)); return e; }
     }
-    pair_h_kernel<<<(unsigned)nblk, PAIR_THREADS, sizeof(PairSmem), st>>>(a);
+    pair_h_kernel<<<(unsigned)nblk, PAIR_THREADS, PairSmemLayout(pl.li, pl.lj).total, st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
