@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmd4.so")
 OBJ = os.path.join(HERE, "build")
-SOURCES = ["md4_api.cu", "md4_pairs.cu", "md4_eri.cu", "md4_tables.cpp"]
+SOURCES = ["md4_api.cu", "md4_pairs.cu", "md4_eri.cu", "md4_eri_small.cu", "md4_tables.cpp"]
 HEADERS = ["md4_internal.h", "md4_device.cuh", os.path.join("..", "..", "include", "md4.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

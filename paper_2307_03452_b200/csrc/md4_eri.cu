@@ -575,6 +575,8 @@ void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows) {
 
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
                       cudaStream_t st, const DigestArgs* dg) {
+    // uncontracted low-l classes: one warp per quartet, no block-level synchronisation (md4_eri_small.cu)
+    if (!dg && small_class_eligible(bra, ket)) return launch_eri_small(ctx, bra, ket, d_out, st);
     EriArgs a;
     a.digest = dg ? 1 : 0;
     a.nbf = dg ? dg->nbf : 0;

@@ -190,6 +190,9 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
                       cudaStream_t st, const DigestArgs* dg = nullptr);
 void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows);   // the work-item split of md4_compute (host logic)
+// md4_eri_small.cu: uncontracted low-l classes, one warp per quartet
+bool small_class_eligible(const PairListDev& bra, const PairListDev& ket);
+md4_status launch_eri_small(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out, cudaStream_t st);
 cudaError_t launch_debug_boys(md4_ctx* ctx, int mmax, int n, const double* d_T, double* d_out);
 cudaError_t launch_debug_r(md4_ctx* ctx, int L, const double* d_pq, double* d_out);
 }  // namespace md4

@@ -616,3 +616,40 @@ def test_k_shell_class_limits(eng):
         assert eng.launch_count() == n0
         bra.free(); ket.free()
     torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------- low angular momenta (S:8(f) item 1)
+@pytest.mark.parametrize("l", [0, 1, 2, 3])
+def test_low_l_full_size_batches(eng, l):
+    """(ss|ss) ... (ff|ff), uncontracted, 64 x 64 = 4096 quartets (the batch size of the sweep): one warp per quartet
+    (md4_eri_small.cu), every warp walks through several quartets.  192 sampled quartets + the first and the last against
+    the binary128 oracle; then the whole batch against the same list computed in 64 single-bra launches (bit-identical:
+    a quartet's arithmetic does not depend on which warp computes it)."""
+    import torch
+
+    wl = inputs._perm_config(f"low l={l}", 11 + l, 64, l, 10.0, 0.05, 50.0, 64)
+    errs, below = _sampled(eng, wl, 192, 300 + l, extra=(0, wl.nquartets - 1))
+    assert errs.max() <= TOL, (l, errs.max())
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    full = eng.compute(bra, ket)
+    torch.cuda.synchronize()
+    for i in range(0, 64, 7):
+        b1 = eng.build_pairs(wl.bra_ij[i:i + 1])
+        one = eng.compute(b1, ket)
+        torch.cuda.synchronize()
+        assert torch.equal(one[0], full[i]), (l, i)
+        b1.free()
+    bra.free(); ket.free()
+
+
+def test_low_l_mixed_and_contracted_classes(eng):
+    """Classes around the boundary of the small-class kernel: mixed low l (one warp per quartet), a contracted low-l class
+    and a low-l bra with a high-l ket (both stay on the fused kernel)."""
+    for lclass, kclass in (((3, 2, 1, 0), (1, 1, 1, 1)), ((3, 3, 2, 2), (1, 1, 1, 1)), ((2, 2, 3, 3), (1, 1, 1, 1)),
+                           ((3, 3, 3, 3), (1, 2, 1, 1)), ((2, 2, 6, 6), (1, 1, 1, 1)), ((6, 6, 2, 1), (1, 1, 1, 1))):
+        wl = inputs.small_workload(lclass, kclass, nbra=5, nket=7, seed=81)
+        g, r = _run(eng, wl)
+        errs, below = _quartet_errors(g, r)
+        assert errs.max() <= TOL, (lclass, kclass, errs.max())
