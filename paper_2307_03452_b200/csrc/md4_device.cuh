@@ -170,16 +170,14 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
 __device__ __forceinline__ void mbar_arrive32(uint32_t bar) {
     asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
 }
-// The same, ordered behind the producers of two values: the arrive is predicated on a comparison of the two (true for
-// every pair of numbers that are not both NaN... it is simply "dep0 == dep0 || dep1 == dep1"), which the assembler can
-// neither evaluate early nor drop, so the arrive cannot be scheduled before both values exist.  If both are NaN the
-// arrive still happens (second instruction): the protocol never loses an arrival.
-__device__ __forceinline__ void mbar_arrive32_after(uint32_t bar, double dep0, double dep1) {
+// arrive that carries a data dependency on `dep`: it is predicated on dep != 0 AND on dep == 0 (two instructions, one of
+// which executes), so the assembler can neither drop `dep` nor schedule the arrive before `dep` has been computed.
+// Used to keep the release of a ring stage behind the completion of every load of the stage (md4_eri.cu).
+__device__ __forceinline__ void mbar_arrive32_dep(uint32_t bar, int dep) {
     asm volatile(
-        "{\n .reg .b64 st;\n .reg .pred p, q;\n"
-        " setp.eq.f64 p, %1, %1;\n setp.eq.or.f64 p, %2, %2, p;\n not.pred q, p;\n"
+        "{\n .reg .b64 st;\n .reg .pred p;\n setp.ne.s32 p, %1, 0;\n"
         " @p mbarrier.arrive.shared::cta.b64 st, [%0];\n"
-        " @q mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(bar), "d"(dep0), "d"(dep1) : "memory");
+        " @!p mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(bar), "r"(dep) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx32(uint32_t bar, uint32_t bytes) {
     asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(bar), "r"(bytes) : "memory");

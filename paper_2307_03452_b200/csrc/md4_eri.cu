@@ -193,6 +193,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
             mbar_wait32(c.full32 + rp.s * 8u, rp.ph);
             const uint32_t bb = c.ring32 + rp.s * c.stage_bytes;
             constexpr int G = 4;   // B fragment pairs in flight
+            int landed = 1;        // becomes data-dependent on every B fragment of the stage (see the release below)
 #pragma unroll
             for (int nb0 = 0; nb0 < NT_CD; nb0 += G) {
                 double2 bv[G];
@@ -205,13 +206,16 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
 #pragma unroll
                 for (int g = 0; g < G; ++g)
                     if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) dmma884(acc[nb0 + g].x, acc[nb0 + g].y, ty, bv[g].y);
+#pragma unroll
+                for (int g = 0; g < G; ++g)
+                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) landed &= (int)(bv[g].y == bv[g].y) | 2;
             }
             __syncwarp();
-            // release the stage.  The arrive takes the last accumulator of the q-block as a (fake) input: it cannot be
-            // scheduled before the last DMMA, i.e. before every B fragment of the stage has been read into registers.
-            // (Without it ptxas places the arrive right behind the ISSUE of the last LDS, ahead of the DMMAs that wait for
-            // the data: the producer may then refill the stage while loads of it are still in flight.)
-            if (c.lane == 0) mbar_arrive32_after(c.empty32 + rp.s * 8u, acc[NT_CD - 1].x, acc[NT_CD - 1].y);
+            // release the stage.  The arrive takes `landed` as an input, a value that depends on every B fragment of the
+            // stage: it cannot be scheduled before all loads of the stage have delivered their data.  (Without it ptxas
+            // places the arrive right behind the ISSUE of the last LDS; the producer may then refill the stage while
+            // loads of it are still in flight -- the write-after-read race of DESIGN.md 6.1.)
+            if (c.lane == 0) mbar_arrive32_dep(c.empty32 + rp.s * 8u, landed);
             rp.advance(c.nst);
         }
     }
