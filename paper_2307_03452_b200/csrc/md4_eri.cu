@@ -193,7 +193,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
             mbar_wait32(c.full32 + rp.s * 8u, rp.ph);
             const uint32_t bb = c.ring32 + rp.s * c.stage_bytes;
             constexpr int G = 4;   // B fragment pairs in flight
-            int landed = 1;        // becomes data-dependent on every B fragment of the stage (see the release below)
+            int landed = 0;        // OR of a word of every B fragment of the stage: unknown to the assembler, see the release below
 #pragma unroll
             for (int nb0 = 0; nb0 < NT_CD; nb0 += G) {
                 double2 bv[G];
@@ -208,7 +208,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
                     if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) dmma884(acc[nb0 + g].x, acc[nb0 + g].y, ty, bv[g].y);
 #pragma unroll
                 for (int g = 0; g < G; ++g)
-                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) landed &= (int)(bv[g].y == bv[g].y) | 2;
+                    if (nb0 + g < NT_CD && (EXACT || nb0 + g < c.nrb_cd)) landed |= __double2loint(bv[g].y);
             }
             __syncwarp();
             // release the stage.  The arrive takes `landed` as an input, a value that depends on every B fragment of the
@@ -455,28 +455,26 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
                 // (a9) 16-byte streaming stores (st.global.cs.v2.f64: the 3.7 GB output stream must not evict H from L2).
                 // A lane holds columns (c, c+1), c = 8 nb + 2 k4, of its row; rows start at element (quartet Nab + row) Ncd of
                 // the output, which is odd for every other row when Ncd is odd: there the aligned pairs are (c+1, c+2), whose
-                // second element comes from the neighbouring lane (or, for k4 = 3, from this row's first lane, next block).
+                // second element comes from the neighbouring lane (one shuffle per block).  One store instruction per block
+                // serves both kinds of rows (address and values selected per lane).
                 const size_t e0 = ((size_t)ib * a.nket + jk) * a.nab * a.ncd + (size_t)(row < a.nab ? row : 0) * a.ncd;
                 double* o = a.out + e0;
-                const bool odd = ((reinterpret_cast<uintptr_t>(o) >> 3) & 1) != 0;   // d_out itself need only be 8-byte aligned
+                const int odd = (int)((reinterpret_cast<uintptr_t>(o) >> 3) & 1);   // d_out itself need only be 8-byte aligned
                 const bool rowok = row < a.nab;
+                const double f2x = (acc[0].x * f) * f;
+                if (rowok && odd && cc.k4 == 0) __stcs(o, f2x);   // first element of a row that starts on an odd element
 #pragma unroll
                 for (int nb = 0; nb < NT_CD; ++nb) {
                     const double vx = (acc[nb].x * f) * f, vy = (acc[nb].y * f) * f;
-                    const double nx_same = __shfl_sync(0xffffffffu, vx, (lane & ~3) | ((cc.k4 + 1) & 3));
-                    double nx_next = 0.0;
-                    if (nb + 1 < NT_CD) nx_next = __shfl_sync(0xffffffffu, (acc[nb + 1].x * f) * f, lane & ~3);
-                    const double nx = cc.k4 == 3 ? nx_next : nx_same;
-                    const int col = nb * 8 + 2 * cc.k4;
+                    // the x value of column c+2: from lane k4+1 (same block) or, for k4 = 3, from the row's lane 0, next block
+                    double sv = vx;
+                    if (nb + 1 < NT_CD && cc.k4 == 0) sv = (acc[nb + 1].x * f) * f;
+                    const double nx = __shfl_sync(0xffffffffu, sv, (lane & ~3) | ((cc.k4 + 1) & 3));
+                    const int c = nb * 8 + 2 * cc.k4 + odd;   // first column of this lane's aligned pair
+                    const double p0 = odd ? vy : vx, p1 = odd ? nx : vy;
                     if (rowok) {
-                        if (!odd) {
-                            if (col + 1 < a.ncd) __stcs(reinterpret_cast<double2*>(o + col), make_double2(vx, vy));
-                            else if (col < a.ncd) __stcs(o + col, vx);
-                        } else {
-                            if (col == 0) __stcs(o, vx);
-                            if (col + 2 < a.ncd) __stcs(reinterpret_cast<double2*>(o + col + 1), make_double2(vy, nx));
-                            else if (col + 1 < a.ncd) __stcs(o + col + 1, vy);
-                        }
+                        if (c + 1 < a.ncd) __stcs(reinterpret_cast<double2*>(o + c), make_double2(p0, p1));
+                        else if (c < a.ncd) __stcs(o + c, p0);
                     }
                 }
             }
