@@ -63,7 +63,7 @@ __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a -
 // additive address per graded ordinal | mbarriers.
 struct SmemLayout {
     size_t ra, un, ga, ss, ap, aq, sg, rt, ad, bars, dg, total, stage_bytes;
-    // digest: D_cd of the ket pair (padded to whole column blocks), D_bd, the K_ac tile of the item, column -> (mc, md)
+    // digest: D_cd of the ket pair (padded to whole column blocks), D_bd, column -> (mc, md)
     static constexpr int DG_TILE = (2 * LMAX + 1) * (2 * LMAX + 1);
     __host__ __device__ SmemLayout(int L, int ncb_p, int ncb_q, int nrb_cd, int nst, int digest = 0) {
         size_t o = 0;
@@ -79,7 +79,7 @@ struct SmemLayout {
         ad = o; o += align_up((size_t)n_hermite(L) * 2, 16);   // additive address per graded ordinal
         bars = o; o += 2 * MAX_STAGES * 8;
         dg = o;
-        if (digest) o += (size_t)nrb_cd * 64 + 2 * DG_TILE * 8 + align_up((size_t)nrb_cd * 8 * 2, 16);
+        if (digest) o += (size_t)nrb_cd * 64 + DG_TILE * 8 + align_up((size_t)nrb_cd * 8 * 2, 16);
         total = o;
     }
 };
@@ -237,8 +237,7 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     uint64_t* empty = full + MAX_STAGES;
     double* sDcd = reinterpret_cast<double*>(smem + lay.dg);          // [nrb_cd * 8]
     double* sDbd = sDcd + a.nrb_cd * 8;                               // [nsb * nsd]
-    double* sK = sDbd + SmemLayout::DG_TILE;                          // [nsa * nsc]
-    uint16_t* cmap = reinterpret_cast<uint16_t*>(sK + SmemLayout::DG_TILE);   // column of cd -> mc << 8 | md
+    uint16_t* cmap = reinterpret_cast<uint16_t*>(sDbd + SmemLayout::DG_TILE);   // column of cd -> mc << 8 | md
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const int L = a.L;
@@ -266,7 +265,6 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     }
     if (a.digest) {
         for (int c = tid; c < a.nrb_cd * 8; c += nthr) cmap[c] = (uint16_t)(c < a.ncd ? ((c / a.nsd) << 8) | (c % a.nsd) : 0);
-        for (int c = tid; c < SmemLayout::DG_TILE; c += nthr) sK[c] = 0.0;
     }
     if (tid == 0) {
         for (int s = 0; s < a.nst; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)a.wpc); }
@@ -315,8 +313,6 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     if (have && producer) build_r(quartet, 0, 0, [] {});
 
     double2 acc[NT_CD];
-    int k_ao_a = 0, k_ao_c = 0;     // digest: AO offsets of the K tile being accumulated in shared memory
-    bool k_pending = false;
     while (have) {
         long long nquartet = quartet;
         int nms = ms, nkq = kq, nkp = kp + 1;
@@ -347,22 +343,12 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
         __syncthreads();  // consumers are done with R of the previous primitive quartet, the builder with GA
         r_scatter(Ra, GA, sad, L, tid, nthr);
         if (a.digest && kq == 0 && kp == 0) {
-            // a new item: the K tile of the previous one goes to the AO matrix (global atomics), then the density blocks
-            // of this quartet are staged: D_cd (for J) and D_bd (for K)
-            const int nsa = a.nab / a.nsb, nsc = a.ncd / a.nsd;
-            if (k_pending) {
-                for (int e = tid; e < nsa * nsc; e += nthr) {
-                    const double v = sK[e];
-                    sK[e] = 0.0;
-                    if (v != 0.0) atomicAdd(a.K + (size_t)(k_ao_a + e / nsc) * a.nbf + k_ao_c + e % nsc, v);
-                }
-            }
+            // a new item: the density blocks of this quartet are staged, D_cd (for J) and D_bd (for K)
             const int ao_b = __ldg(a.aob + 2 * ib + 1), ao_c = __ldg(a.aok + 2 * jk), ao_d = __ldg(a.aok + 2 * jk + 1);
             for (int c = tid; c < a.nrb_cd * 8; c += nthr)
                 sDcd[c] = c < a.ncd ? __ldg(a.D + (size_t)(ao_c + c / a.nsd) * a.nbf + ao_d + c % a.nsd) : 0.0;
             for (int e = tid; e < a.nsb * a.nsd; e += nthr)
                 sDbd[e] = __ldg(a.D + (size_t)(ao_b + e / a.nsd) * a.nbf + ao_d + e % a.nsd);
-            k_ao_a = __ldg(a.aob + 2 * ib); k_ao_c = ao_c; k_pending = true;
         }
         __syncthreads();
 
@@ -415,40 +401,68 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
             // correctly rounded
             if (item_ends && a.digest) {
                 // ---- direct digestion: the row's (ab|cd) values meet D_cd (Coulomb-type J, one number per
-                // row after a reduction over the four lanes of the row) and D_bd (exchange-type K, accumulated per (ma, mc)
-                // in the shared-memory tile); nothing is stored per quartet
+                // row after a reduction over the four lanes of the row) and D_bd (exchange-type K, summed per (ma, mc) by a
+                // small DMMA and a segmented reduction over the rows); nothing is stored per quartet
                 const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
-                const int row = mbk * 8 + (lane >> 2);
+                const int nrow = lane >> 2;
+                const int row = mbk * 8 + nrow;
                 const bool rowok = row < a.nab;
-                const int ma = rowok ? row / a.nsb : 0, mb = rowok ? row % a.nsb : 0;
+                const int ma = row / a.nsb, mb = rowok ? row % a.nsb : 0;   // rows of the padding have ma >= 2 l_a + 1 and zero values
                 const int nsc = a.ncd / a.nsd;
-                double js = 0.0, ks = 0.0;
-                int cur = -1;
+                double js = 0.0;
+                double2 S0 = make_double2(0.0, 0.0), S1 = make_double2(0.0, 0.0);   // S[row][mc]: mc = 2 k4 (+1), 8 + 2 k4 (+1)
 #pragma unroll
                 for (int nb = 0; nb < NT_CD; ++nb) {
+                    if (!EXACT && nb >= a.nrb_cd) break;
                     const int col = nb * 8 + 2 * cc.k4;
-                    const double vx = (acc[nb].x * f) * f, vy = (acc[nb].y * f) * f;
+                    const double vx = rowok ? (acc[nb].x * f) * f : 0.0, vy = rowok ? (acc[nb].y * f) * f : 0.0;
                     js = fma(vx, sDcd[col], fma(vy, sDcd[col + 1], js));
                     if (a.K) {
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const int c = col + h;
-                            if (c < a.ncd && rowok) {
-                                const int w = cmap[c], mc = w >> 8, md = w & 255;
-                                if (mc != cur) {
-                                    if (cur >= 0) atomicAdd(sK + ma * nsc + cur, ks);
-                                    cur = mc; ks = 0.0;
-                                }
-                                ks = fma(h ? vy : vx, sDbd[mb * a.nsd + md], ks);
-                            }
+                        // K: weight every value with D[b, d], then sum the md index on the tensor pipe: S += W . B with
+                        // B[column][mc] = 1 where the column belongs to mc.  W is in C-fragment layout, which is the
+                        // A-fragment layout of the two k-steps (as in GEMM2); lane (k4, nrow) makes B[k = k4][n = nrow]
+                        // from the column -> (mc, md) map of its own two columns.
+                        const int wx = cmap[col], wy = cmap[col + 1];
+                        const double ax = vx * sDbd[mb * a.nsd + (wx & 255)], ay = vy * sDbd[mb * a.nsd + (wy & 255)];
+                        const int mcx = wx >> 8, mcy = wy >> 8;
+                        dmma884(S0.x, S0.y, ax, mcx == nrow ? 1.0 : 0.0);
+                        dmma884(S0.x, S0.y, ay, mcy == nrow ? 1.0 : 0.0);
+                        if (nsc > 8) {
+                            dmma884(S1.x, S1.y, ax, mcx == nrow + 8 ? 1.0 : 0.0);
+                            dmma884(S1.x, S1.y, ay, mcy == nrow + 8 ? 1.0 : 0.0);
                         }
                     }
                 }
-                if (a.K && cur >= 0) atomicAdd(sK + ma * nsc + cur, ks);
                 js += __shfl_xor_sync(0xffffffffu, js, 1);
                 js += __shfl_xor_sync(0xffffffffu, js, 2);
+                const int ao_a = __ldg(a.aob + 2 * ib);
                 if (a.J && rowok && cc.k4 == 0)
-                    atomicAdd(a.J + (size_t)(__ldg(a.aob + 2 * ib) + ma) * a.nbf + __ldg(a.aob + 2 * ib + 1) + mb, js);
+                    atomicAdd(a.J + (size_t)(ao_a + ma) * a.nbf + __ldg(a.aob + 2 * ib + 1) + mb, js);
+                if (a.K) {
+                    // sum over the rows that share ma (rows are sorted by ma: segmented suffix sums by doubling), then the
+                    // first row of every segment adds its four (ma, mc) sums to the AO matrix
+                    double v[4] = {S0.x, S0.y, S1.x, S1.y};
+#pragma unroll
+                    for (int d = 1; d < 8; d *= 2) {
+                        const int ma_o = __shfl_down_sync(0xffffffffu, ma, 4 * d);
+                        const bool take = nrow + d < 8 && ma_o == ma;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const double o = __shfl_down_sync(0xffffffffu, v[i], 4 * d);
+                            if (take) v[i] += o;
+                        }
+                    }
+                    const int ma_p = __shfl_up_sync(0xffffffffu, ma, 4);
+                    const bool head = nrow == 0 || ma_p != ma;
+                    if (head && rowok) {
+                        double* Kr = a.K + (size_t)(ao_a + ma) * a.nbf + __ldg(a.aok + 2 * jk);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const int mc = (i >> 1) * 8 + 2 * cc.k4 + (i & 1);
+                            if (mc < nsc && v[i] != 0.0) atomicAdd(Kr + mc, v[i]);
+                        }
+                    }
+                }
             } else if (item_ends) {
                 const double f = exp(0.5 * (__ldg(a.pmb + ib) + __ldg(a.pmk + jk)));
                 const int row = mbk * 8 + (lane >> 2);
@@ -480,14 +494,6 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
             }
         }
         quartet = nquartet; ms = nms; kq = nkq; kp = nkp; have = nhave;
-    }
-    if (a.digest && k_pending) {
-        __syncthreads();
-        const int nsa = a.nab / a.nsb, nsc = a.ncd / a.nsd;
-        for (int e = tid; e < nsa * nsc; e += nthr) {
-            const double v = sK[e];
-            if (v != 0.0) atomicAdd(a.K + (size_t)(k_ao_a + e / nsc) * a.nbf + k_ao_c + e % nsc, v);
-        }
     }
 }
 
