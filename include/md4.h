@@ -133,6 +133,26 @@ md4_status md4_output_size(const md4_pairs* bra, const md4_pairs* ket, size_t* n
 md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out,
                        size_t capacity_doubles, void* cuda_stream);
 
+/* md4_compute for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same result (bit for bit the same kernel), but the one scratch the
+ * fused kernel uses -- the partial sums [ab|q~] of CONTRACTED bras (Listing 2.1 line 7), parked between bra
+ * primitives -- lives in a file-scope `static __device__` array of MD4_STATIC_SCRATCH_BYTES inside the library instead
+ * of the context's own buffer.  The call itself (and everything it calls) allocates nothing on the device: no
+ * cudaMalloc, cudaFree or allocating library routine; the pair lists are inputs built beforehand (md4_build_pairs).
+ *   - Every GPU that loads libmd4.so holds the array (32 MiB) until the process exits.
+ *   - A contracted bra class whose launch needs more (num_SMs x resident CTAs x consumer warps x q~ column blocks x 512
+ *     bytes: e.g. (ii|ii), (ih|ih) at K > 1 on 148 SMs) is rejected with MD4_EUNSUPPORTED and a message that names both
+ *     numbers; nothing is enqueued.  Uncontracted bras (K_a = K_b = 1) use no scratch and are never rejected for size.
+ *   - All calls on a device share the array, across contexts and streams, and it keeps the last call's contents.  The
+ *     kernel writes every slot before it reads it, so nothing needs clearing between calls -- but two calls with
+ *     contracted bras that OVERLAP on the GPU (different streams, different contexts, different host threads) race on
+ *     it and give wrong integrals: the caller serialises them (one stream, or events).  md4_compute does not use the
+ *     array and may overlap with one md4_compute_static.
+ * Other errors, ordering against the pair builds and the output layout as for md4_compute. */
+#define MD4_STATIC_SCRATCH_BYTES (32u * 1024u * 1024u)
+md4_status md4_compute_static(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out,
+                              size_t capacity_doubles, void* cuda_stream);
+
 /* Same through HOST buffers (the end-to-end path bench.py's "e2e" times): copies the result to
  * h_out [capacity_doubles] (HOST) through an internal device buffer that grows on demand, and
  * synchronises before returning.  Large batches are computed in slices of the bra list; the copy of a slice

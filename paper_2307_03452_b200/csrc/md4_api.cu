@@ -499,6 +499,33 @@ md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket,
     return MD4_OK;
 }
 
+// md4_compute with the [ab|q~] scratch in the library's static device array (md4_eri.cu: launch_eri_static).  Ordering:
+// the launch waits for the pair kernels of both lists and the lists remember it as their last reader, as in
+// md4_compute; the static scratch itself is NOT ordered (shared by every context on the device, md4.h).
+md4_status md4_compute_static(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* d_out,
+                              size_t capacity_doubles, void* cuda_stream) {
+    size_t need = 0;
+    md4_status s = check_compute(ctx, bra, ket, d_out, capacity_doubles, &need);
+    if (s != MD4_OK || need == 0) return s;
+    DeviceGuard g(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaStreamWaitEvent(st, bra->ready, 0);
+    if (e == cudaSuccess && ket != bra) e = cudaStreamWaitEvent(st, ket->ready, 0);
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_static", e);
+    s = launch_eri_static(ctx, bra->d, ket->d, d_out, st);
+    if (s != MD4_OK) return s;
+    md4_pairs* b = const_cast<md4_pairs*>(bra);
+    md4_pairs* k = const_cast<md4_pairs*>(ket);
+    if (b->used) e = cudaStreamWaitEvent(st, b->last_use, 0);
+    if (e == cudaSuccess) { e = cudaEventRecord(b->last_use, st); b->used = true; }
+    if (e == cudaSuccess && k != b) {
+        if (k->used) e = cudaStreamWaitEvent(st, k->last_use, 0);
+        if (e == cudaSuccess) { e = cudaEventRecord(k->last_use, st); k->used = true; }
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute_static", e);
+    return MD4_OK;
+}
+
 md4_status md4_compute_host(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket, double* h_out,
                             size_t capacity_doubles, void* cuda_stream) {
     size_t need = 0;

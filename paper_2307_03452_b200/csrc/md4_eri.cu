@@ -22,6 +22,8 @@
 // no f64 kind on sm_100a, S: facts table).  (ab|cd) accumulates in registers over all primitive
 // quartets (Listing 2.1) and is written once.
 #include "md4_device.cuh"
+#include <mutex>
+#include <string>
 
 namespace md4 {
 
@@ -581,8 +583,10 @@ void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows) {
     for (int t = 0; t < 3; ++t) { row0[t] = a.row0[t]; nrows[t] = a.nrows[t]; }
 }
 
-md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
-                      cudaStream_t st, const DigestArgs* dg) {
+// tacc: the [ab|q~] scratch of contracted bras; tacc_cap: its size in bytes, checked against what the launch can touch
+// (0: the context's own scratch, sized for every class at md4_create)
+static md4_status launch_eri_with(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
+                                  cudaStream_t st, const DigestArgs* dg, double* tacc, size_t tacc_cap) {
     // uncontracted low-l classes: one warp per quartet, no block-level synchronisation (md4_eri_small.cu)
     if (!dg && small_class_eligible(bra, ket)) return launch_eri_small(ctx, bra, ket, d_out, st);
     EriArgs a;
@@ -617,8 +621,19 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     a.ks = ctx->kernel;
     a.colp = ctx->tab.colb[bra.lsum]; a.colq = ctx->tab.colk[ket.lsum];
     a.out = d_out;
-    a.tacc = ctx->d_tacc;
+    a.tacc = tacc;
     const int nt = a.nrb_cd;
+    if (tacc_cap && a.Kb > 1) {
+        // one slab of wpc x ncb_q fragment blocks (512 bytes each) per CTA; resident CTAs per SM as in launch_small
+        const int minb = nt <= 7 ? (a.wpc + 1 <= 4 ? 3 : (a.wpc + 1 <= 8 ? 2 : 1)) : 1;
+        const size_t need = (size_t)ctx->num_sms * minb * a.wpc * a.ncb_q * 64 * sizeof(double);
+        if (need > tacc_cap) {
+            ctx->err = "md4_compute_static: this contracted bra class needs " + std::to_string(need) +
+                       " bytes of [ab|q~] scratch, the static scratch holds " + std::to_string(tacc_cap) +
+                       " (MD4_STATIC_SCRATCH_BYTES); use md4_compute";
+            return MD4_EUNSUPPORTED;
+        }
+    }
     // exact instantiations for the ket classes of l >= 4 shells (N_cd = 81, 99, 117, 121, 143, 169); the
     // others (no product of two odd numbers <= 13 falls in 14, 17, 19-21 row blocks) run predicated
     if (nt == 11) return launch_w<11, true>(ctx, a, st);
@@ -634,6 +649,48 @@ md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& k
     if (nt <= 22) return launch_w<22, false>(ctx, a, st);   // kets with an l = 7 shell: 15 x 9 = 135 (17 blocks), 15 x 11 = 165 (21)
     ctx->err = "md4_compute: ket class too large";
     return MD4_EUNSUPPORTED;
+}
+
+md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
+                      cudaStream_t st, const DigestArgs* dg) {
+    return launch_eri_with(ctx, bra, ket, d_out, st, dg, ctx->d_tacc, 0);
+}
+
+// ---- md4_compute_static: the fused kernel with its [ab|q~] scratch in a file-scope device array ---------------------
+// For callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  The array is
+// part of the library image: every GPU that loads libmd4.so holds MD4_STATIC_SCRATCH_BYTES until the process exits.  All
+// calls on a device share it, whatever the context; it keeps the last call's contents.  Nothing in it has to start at
+// zero: a CTA stores the partial [ab|q~] of a bra primitive before it loads it for the next one (consume_chunk), so there
+// is nothing to clear -- but two launches with contracted bras that overlap on the GPU race on it.
+namespace {
+static __device__ __align__(256) double md4_static_tacc[MD4_STATIC_SCRATCH_BYTES / sizeof(double)];
+constexpr int STATIC_MAX_DEVICES = 64;
+double* g_static_tacc[STATIC_MAX_DEVICES] = {};   // device address of the array, per device ordinal (looked up once)
+std::mutex g_static_mu;
+}  // namespace
+
+md4_status launch_eri_static(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out, cudaStream_t st) {
+    // In host code `md4_static_tacc` is a host-side stand-in, not a device address: ask the runtime for the address on
+    // the current device (the caller has made ctx->device current) and pass that to the kernel.
+    if (ctx->device < 0 || ctx->device >= STATIC_MAX_DEVICES) {
+        ctx->err = "md4_compute_static: device ordinal beyond 63";
+        return MD4_EUNSUPPORTED;
+    }
+    double* tacc = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        if (!g_static_tacc[ctx->device]) {
+            void* p = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress(&p, md4_static_tacc);
+            if (e != cudaSuccess) {
+                ctx->err = std::string("md4_compute_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e);
+                return MD4_ECUDA;
+            }
+            g_static_tacc[ctx->device] = static_cast<double*>(p);
+        }
+        tacc = g_static_tacc[ctx->device];
+    }
+    return launch_eri_with(ctx, bra, ket, d_out, st, nullptr, tacc, (size_t)MD4_STATIC_SCRATCH_BYTES);
 }
 
 // ---- stage-level debug kernels ---------------------------------------------------------------------

@@ -189,6 +189,8 @@ cudaError_t launch_pair_kernel(md4_ctx* ctx, const PairListDev& pl, cudaStream_t
 // md4_eri.cu
 md4_status launch_eri(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out,
                       cudaStream_t st, const DigestArgs* dg = nullptr);
+// same, with the [ab|q~] scratch of contracted bras in the library's file-scope device array (md4_compute_static)
+md4_status launch_eri_static(md4_ctx* ctx, const PairListDev& bra, const PairListDev& ket, double* d_out, cudaStream_t st);
 void plan_items_host(int nrb_ab, int* nitems, int* row0, int* nrows);   // the work-item split of md4_compute (host logic)
 // md4_eri_small.cu: uncontracted low-l classes, one warp per quartet
 bool small_class_eligible(const PairListDev& bra, const PairListDev& ket);

@@ -22,7 +22,7 @@ STATUS_NAMES = ["MD4_OK", "MD4_EINVAL", "MD4_EUNSUPPORTED", "MD4_ESTATE", "MD4_E
 SYMBOLS = [
     "md4_create", "md4_destroy", "md4_last_error", "md4_set_shells", "md4_build_pairs", "md4_free_pairs",
     "md4_stream_wait_pairs", "md4_set_kernel", "md4_num_ao", "md4_compute_jk", "md4_compute_jk_host",
-    "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host",
+    "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host", "md4_compute_static",
     "md4_launch_count", "md4_flops_per_quartet", "md4_debug_boys", "md4_debug_solid_coeff",
     "md4_debug_hermite_r", "md4_debug_pair_h", "md4_debug_work_items",
 ]
@@ -71,6 +71,8 @@ def load():
     lib.md4_compute.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, vp]
     lib.md4_compute.restype = ctypes.c_int
     lib.md4_compute_host.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, vp]
+    lib.md4_compute_static.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, vp]
+    lib.md4_compute_static.restype = ctypes.c_int
     lib.md4_compute_host.restype = ctypes.c_int
     lib.md4_num_ao.argtypes = [vp, ip]
     lib.md4_num_ao.restype = ctypes.c_int
@@ -213,6 +215,20 @@ class Engine:
             stream = torch.cuda.current_stream(self.device).cuda_stream
         self._check(load().md4_compute(self.handle, bra.handle, ket.handle, ctypes.c_void_p(out.data_ptr()),
                                        out.numel(), ctypes.c_void_p(stream)))
+        return out.view(-1)[:n].view(self.output_shape(bra, ket)) if n else out.view(-1)[:0]
+
+    def compute_static(self, bra: PairList, ket: PairList, out, stream=None):
+        """Enqueue md4_compute_static (no device allocation: the [ab|q~] scratch of contracted bras is the library's static
+        32 MiB device array, md4.h) into the caller's contiguous float64 CUDA tensor ``out``; returns it shaped like compute."""
+        import torch
+
+        n = self.output_size(bra, ket)
+        if out.dtype != torch.float64 or not out.is_cuda or not out.is_contiguous():
+            raise ValueError("out must be a contiguous float64 CUDA tensor")
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        self._check(load().md4_compute_static(self.handle, bra.handle, ket.handle, ctypes.c_void_p(out.data_ptr()),
+                                              out.numel(), ctypes.c_void_p(stream)))
         return out.view(-1)[:n].view(self.output_shape(bra, ket)) if n else out.view(-1)[:0]
 
     def compute_ptr(self, bra: PairList, ket: PairList, d_ptr: int, capacity: int, stream: int = 0):
