@@ -148,22 +148,26 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
     // for hh / ig kets (+4 %; 2 warps per sub-partition, so a k-block passes in ~1 us), costs 7 % for gg kets (short
     // k-loops, long prologue) and 3 % for ii kets (no registers to spare)
     constexpr int PF = (NT_CD == 15 || NT_CD == 16) ? PF_SMALL : PF_LARGE;
+    // The address of the fragment PF k-blocks ahead is a running pointer (2 instructions per k-block; indexing it as
+    // Ablk[(jb + PF) * astride] compiled to a 64-bit multiply-add chain of 7 and cost 3 % of the kernel: three warps per
+    // sub-partition issue ~4 instructions per 16-clock DMMA each, the issue port is the second bottleneck).  The load stays
+    // predicated: unconditional loads (into slack behind the list) save 4 moves per k-block but make the assembler hoist
+    // them and spill accumulators (measured: 55.2-57.3 ms against 54.7 on cfg3).
     double2 af[PF];
 #pragma unroll
     for (int i = 0; i < PF; ++i) af[i] = i < c.ncb_p ? ldg2(c.Ablk + (size_t)i * c.astride) : make_double2(0.0, 0.0);
-    int2 apn = lds_v2s32(c.ap32);
+    const double* apf = c.Ablk + (size_t)PF * c.astride;
+    uint32_t app32 = c.ap32;
+    int2 apn = lds_v2s32(app32);
     for (int jb = 0; jb < c.ncb_p; ++jb) {
         const double2 av = af[0];
-        if constexpr (PF == 2) {
-            af[0] = af[1];
-            if (jb + 2 < c.ncb_p) af[1] = ldg2(c.Ablk + (size_t)(jb + 2) * c.astride);
-        } else {
 #pragma unroll
-            for (int i = 0; i + 1 < PF; ++i) af[i] = af[i + 1];
-            if (jb + PF < c.ncb_p) af[PF - 1] = ldg2(c.Ablk + (size_t)(jb + PF) * c.astride);
-        }
+        for (int i = 0; i + 1 < PF; ++i) af[i] = af[i + 1];
+        if (jb + PF < c.ncb_p) af[PF - 1] = ldg2(apf);
+        apf += c.astride;
         const int2 app = apn;
-        apn = lds_v2s32(c.ap32 + (uint32_t)(jb + 1) * 32u);   // the ap array has one block of slack
+        app32 += 32u;
+        apn = lds_v2s32(app32);   // the ap array has one block of slack
         double b[NQ];
 #pragma unroll
         for (int n = 0; n < NQ; ++n)
