@@ -30,12 +30,16 @@ namespace md4 {
 namespace {
 
 constexpr int MAX_STAGES = 16;
-#ifndef PF_SMALL
-#define PF_SMALL 6
-#endif
-#ifndef PF_LARGE
-#define PF_LARGE 2
-#endif
+
+// How many k-blocks ahead GEMM1 loads its H_ab fragments (16 bytes per lane and k-block, from L2), per kernel
+// instantiation: MAXW = 9 are the bras with at most 8 row blocks per item (hg, hh, ig: two consumer warps per
+// sub-partition), MAXW = 12 those with 10-11 (gg, ih, ii: three); nt = 8-column blocks of the ket.  Measured on the 21
+// classes of cfg5 (K = 1) with depths 1, 2, 4, 5 in every slot; every extra k-block costs 4 registers and 4 moves per
+// k-block, and the differences are 0-9 % (e.g. (hh|hh) 4.76 / 5.23 / 4.81 / 4.80 ms, (ih|ih) 7.91 / 8.17 / 8.02 / 8.17 ms).
+__host__ __device__ constexpr int pf_depth(int maxw, int nt) {
+    if (maxw <= 9) return nt == 13 ? 4 : ((nt == 11 || nt == 15 || nt == 16) ? 1 : 2);
+    return (nt == 15 || nt == 16) ? 5 : (nt == 18 ? 1 : 2);
+}
 
 struct EriArgs {
     const double* Hb; const double* sb; const double* pmb; size_t hsb;
@@ -130,7 +134,7 @@ struct ConsumerCtx {
 // One chunk of NQ q~ blocks for one warp: T = H_ab[8 rows] . G[:, chunk] (GEMM1), then
 // acc += (sign . T) . H_cd[:, chunk]^T (GEMM2) against the ring.  PRED: q-blocks n >= nq are skipped
 // (general classes); otherwise nq == NQ.  EXACT: nrb_cd == NT_CD.
-template <int NQ, int NT_CD, bool EXACT, bool PRED>
+template <int NQ, int NT_CD, bool EXACT, bool PRED, int PF>
 __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const ConsumerCtx& c, int j0, int nq, RingPos& rp,
                                               bool load_t, bool last_kp) {
     double2 T[NQ];
@@ -144,10 +148,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
         aqr[n] = c.ra32 + ((!PRED || n < nq) ? lds_u32(c.aq32 + (uint32_t)(j0 + n) * 32u) : 0u);
     }
     // ---- GEMM1: the B operand is G[p~,q~] = +-R[p~+q~] read at address(p~) + address(q~) (Eq.8)
-    // H_ab fragments come from L2 (~1 us), PF k-blocks ahead.  Measured per ket class (profiles/r1_sweep.md): 6 pays
-    // for hh / ig kets (+4 %; 2 warps per sub-partition, so a k-block passes in ~1 us), costs 7 % for gg kets (short
-    // k-loops, long prologue) and 3 % for ii kets (no registers to spare)
-    constexpr int PF = (NT_CD == 15 || NT_CD == 16) ? PF_SMALL : PF_LARGE;
+    // H_ab fragments come from L2 (~1 us), PF k-blocks ahead (pf_depth above).
     // The address of the fragment PF k-blocks ahead is a running pointer (2 instructions per k-block; indexing it as
     // Ablk[(jb + PF) * astride] compiled to a 64-bit multiply-add chain of 7 and cost 3 % of the kernel: three warps per
     // sub-partition issue ~4 instructions per 16-clock DMMA each, the issue port is the second bottleneck).  The load stays
@@ -279,6 +280,7 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     __syncthreads();
 
     const int nchunk = (a.ncb_q + NQT - 1) / NQT;
+    constexpr int PF = pf_depth(MAXW, NT_CD);
     ConsumerCtx cc;
     cc.astride = (size_t)a.nrb_ab * 64;
     cc.ra32 = smem_u32(Ra);
@@ -398,9 +400,9 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
             for (int ch = 0; ch < nchunk; ++ch) {
                 const int j0 = ch * a.ncb_q / nchunk;
                 const int nq = (ch + 1) * a.ncb_q / nchunk - j0;
-                if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false>(acc, cc, j0, nq, rp, kp > 0, last_kp);
-                else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false>(acc, cc, j0, nq, rp, kp > 0, last_kp);
-                else consume_chunk<NQT - 2, NT_CD, EXACT, true>(acc, cc, j0, nq, rp, kp > 0, last_kp);
+                if (nq == NQT) consume_chunk<NQT, NT_CD, EXACT, false, PF>(acc, cc, j0, nq, rp, kp > 0, last_kp);
+                else if (nq == NQT - 1) consume_chunk<NQT - 1, NT_CD, EXACT, false, PF>(acc, cc, j0, nq, rp, kp > 0, last_kp);
+                else consume_chunk<NQT - 2, NT_CD, EXACT, true, PF>(acc, cc, j0, nq, rp, kp > 0, last_kp);
             }
             // ---- epilogue after the last primitive quartet of the item: common factor K_ab K_cd of the pair
             // maxima, applied in two halves so that results near the bottom of the FP64 range are still
