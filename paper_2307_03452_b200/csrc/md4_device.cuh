@@ -71,11 +71,22 @@ __device__ __forceinline__ double kernel_seed(const double* __restrict__ boys, c
 // every value (K_ab K_cd relative to the pair maxima; 1 in the debug kernel).
 __host__ __device__ inline int r_graded_alloc(int L) { return n_hermite(L) + L; }
 
-template <class Poll>
+// GS = 32 (one warp, `gtid` = lane) or a multiple of 32: then the builder warps of the fused kernel share the elements of
+// every batch (thread gtid of gsize) and meet at named barrier 1 where the one-warp version has a __syncwarp; the batches
+// are gsize * B elements.  The argument above holds between warps as well: a warp that runs ahead into the next (lower)
+// batch only loads elements of lower ordinals than anything the batch above stores over.
+template <int GS>
+__device__ __forceinline__ void r_group_sync() {
+    if constexpr (GS == 32) __syncwarp();
+    else asm volatile("bar.sync 1, %0;\n" ::"n"(GS) : "memory");
+}
+
+template <int GS = 32, class Poll>
 __device__ __forceinline__ void hermite_r_warp(double* G, double* sS, const uint32_t* srt,
                                                const double* __restrict__ boys, const KernelSpec& ks, int L, double zp, double Px,
                                                double Py, double Pz, double zq, double Qx, double Qy, double Qz,
-                                               double scale, int lane, Poll poll) {
+                                               double scale, int gtid, Poll poll) {
+    constexpr int gsize = GS;
     const double X0 = Px - Qx, X1 = Py - Qy, X2 = Pz - Qz;
     {
         const double zs = zp + zq;
@@ -83,29 +94,29 @@ __device__ __forceinline__ void hermite_r_warp(double* G, double* sS, const uint
         const double T = rho * (X0 * X0 + X1 * X1 + X2 * X2);
         // 2 pi^{5/2} = 34.98683665524972497
         const double pref = scale * 34.986836655249724970 / (zp * zq * sqrt(zs));
-        if (lane <= L) {
-            const double F = kernel_seed(boys, ks, lane, rho, T);
+        if (gtid <= L) {
+            const double F = kernel_seed(boys, ks, gtid, rho, T);
             double pw = pref;
             const double m2r = -2.0 * rho;
-            for (int k = 0; k < lane; ++k) pw *= m2r;
-            sS[lane] = pw * F;
+            for (int k = 0; k < gtid; ++k) pw *= m2r;
+            sS[gtid] = pw * F;
         }
     }
-    __syncwarp();
-    if (lane == 0) G[L] = sS[L];   // level 0: [0]^(L)
-    __syncwarp();
-    constexpr int B = 4;  // independent elements in flight per lane
+    r_group_sync<GS>();
+    if (gtid == 0) G[L] = sS[L];   // level 0: [0]^(L)
+    r_group_sync<GS>();
+    constexpr int B = 4;  // independent elements in flight per thread
     for (int l = 1; l <= L; ++l) {
         const int n = n_hermite(l);
         const double* src = G + (L - l + 1);
         double* dst = G + (L - l);
-        const int nbatch = (n + 32 * B - 1) / (32 * B);
+        const int nbatch = (n + gsize * B - 1) / (gsize * B);
         for (int bt = nbatch - 1; bt >= 0; --bt) {
-            const int e0 = bt * 32 * B + lane;
+            const int e0 = bt * gsize * B + gtid;
             uint32_t w[B];
 #pragma unroll
             for (int k = 0; k < B; ++k) {
-                const int e = e0 + k * 32;
+                const int e = e0 + k * gsize;
                 w[k] = srt[e < n ? e : n - 1];
             }
             double val[B];
@@ -115,16 +126,16 @@ __device__ __forceinline__ void hermite_r_warp(double* G, double* sS, const uint
                 const double x = ax == 0 ? X0 : (ax == 1 ? X1 : X2);
                 val[k] = fma((double)((w[k] >> 24) & 31), src[w[k] & 4095], x * src[(w[k] >> 12) & 4095]);
             }
-            __syncwarp();   // every load of the batch precedes its stores
+            r_group_sync<GS>();   // every load of the batch precedes its stores
 #pragma unroll
             for (int k = 0; k < B; ++k) {
-                const int e = e0 + k * 32;
+                const int e = e0 + k * gsize;
                 if (e == 0) val[k] = sS[L - l];
                 if (e < n) dst[e] = val[k];
             }
             poll();
         }
-        __syncwarp();
+        r_group_sync<GS>();
     }
 }
 

@@ -31,13 +31,24 @@ namespace {
 
 constexpr int MAX_STAGES = 16;
 
+// Kernel instantiations by MAXW: 12 = bras with 10-11 row blocks per item (gg, ih, ii: three consumer warps per
+// sub-partition) + 1 producer warp; 10 = bras with 8 row blocks per item (hh, ig: two consumer warps per sub-partition) + 4
+// warps that build R, one per sub-partition; 9 = bras with up to 7 (hg: 7 + 6) + 1 producer warp, which then sits on the
+// sub-partition with one consumer warp; 8 / 4 = small classes, 2 / 3 CTAs per SM.  Registers are allocated per 4 warps, so
+// the 12 warps of MAXW = 10 cost no more than 9 (168 registers either way).
+// Why 4 builders: one producer warp took 6 % from the two consumer warps it shared a sub-partition with, and the other six
+// waited for those two at the block barrier; spread over the four sub-partitions the same work costs every warp 1.5 %
+// ((hh|gg) 2.90 -> 2.52 ms, (hh|hg) 3.80 -> 3.48, (ig|ig) 4.75 -> 4.53).
+__host__ __device__ constexpr int builder_warps(int maxw) { return maxw == 10 ? 4 : 1; }
+__host__ __device__ constexpr int cta_warps_max(int maxw) { return maxw == 10 ? 12 : maxw; }
+
 // How many k-blocks ahead GEMM1 loads its H_ab fragments (16 bytes per lane and k-block, from L2), per kernel
-// instantiation: MAXW = 9 are the bras with at most 8 row blocks per item (hg, hh, ig: two consumer warps per
-// sub-partition), MAXW = 12 those with 10-11 (gg, ih, ii: three); nt = 8-column blocks of the ket.  Measured on the 21
-// classes of cfg5 (K = 1) with depths 1, 2, 4, 5 in every slot; every extra k-block costs 4 registers and 4 moves per
-// k-block, and the differences are 0-9 % (e.g. (hh|hh) 4.76 / 5.23 / 4.81 / 4.80 ms, (ih|ih) 7.91 / 8.17 / 8.02 / 8.17 ms).
+// instantiation; nt = 8-column blocks of the ket.  Measured on the 21 classes of cfg5 (K = 1) with depths 1, 2, 4, 5 in
+// every slot; every extra k-block costs 4 registers and 4 moves per k-block, and the differences are 0-9 % (e.g. (ih|ih)
+// 7.91 / 8.17 / 8.02 / 8.17 ms, (hh|hh) with four builders 4.70 / 5.03 / 4.62 / - ms).
 __host__ __device__ constexpr int pf_depth(int maxw, int nt) {
-    if (maxw <= 9) return nt == 13 ? 4 : ((nt == 11 || nt == 15 || nt == 16) ? 1 : 2);
+    if (maxw == 10) return nt == 11 ? 1 : ((nt == 13 || nt == 15 || nt == 16) ? 4 : 2);
+    if (maxw <= 9) return (nt == 11 || nt == 13) ? 4 : 2;
     return (nt == 15 || nt == 16) ? 5 : (nt == 18 ? 1 : 2);
 }
 
@@ -229,7 +240,7 @@ __device__ __forceinline__ void consume_chunk(double2 (&acc)[NT_CD], const Consu
 }
 
 template <int NT_CD, int NQT, int MAXW, bool EXACT, int MINB>
-__global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
+__global__ void __launch_bounds__(cta_warps_max(MAXW) * 32, MINB) eri_kernel(const EriArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     const SmemLayout lay(a.L, a.ncb_p, a.ncb_q, a.nrb_cd, a.nst, a.digest);
     double* Ra = reinterpret_cast<double*>(smem + lay.ra);
@@ -300,6 +311,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     const uint32_t ringbase32 = smem_u32(smem + lay.un);
     RingPos rp{0u, 0u};  // same sequence in every warp
     const bool producer = (warp == a.wpc);
+    constexpr int NBW = builder_warps(MAXW);
+    const bool helper = NBW > 1 && warp > a.wpc;   // further R-builder warps (a.nbw - 1 of them), one per sub-partition
 
     // builds R of primitive quartet (it, q, p) into GA; poll() is called between batches
     auto build_r = [&](long long it, int q, int p, auto poll) {
@@ -307,8 +320,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
         quartet_pairs(a, it, ib, jk);
         const double* sp = a.sb + ((size_t)ib * a.Kb + p) * 8;
         const double* sq = a.sk + ((size_t)jk * a.Kk + q) * 8;
-        hermite_r_warp(GA, sS, srt, a.boys, a.ks, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
-                       __ldg(sq + 1), __ldg(sq + 2), __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), lane, poll);
+        hermite_r_warp<NBW * 32>(GA, sS, srt, a.boys, a.ks, L, __ldg(sp), __ldg(sp + 1), __ldg(sp + 2), __ldg(sp + 3), __ldg(sq),
+                       __ldg(sq + 1), __ldg(sq + 2), __ldg(sq + 3), exp(__ldg(sp + 4) + __ldg(sq + 4)), (warp - a.wpc) * 32 + lane, poll);
     };
 
     // primitive quartets of this CTA in order: (quartet, item of the quartet, kq, kp), kp fastest.  A CTA takes
@@ -318,7 +331,7 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
     int ms = a.qmajor ? 0 : (int)(blockIdx.x % a.ncta_per_q);
     int kq = 0, kp = 0;
     bool have = quartet < a.nquartets;
-    if (have && producer) build_r(quartet, 0, 0, [] {});
+    if (have && (producer || helper)) build_r(quartet, 0, 0, [] {});
 
     double2 acc[NT_CD];
     while (have) {
@@ -386,6 +399,8 @@ __global__ void __launch_bounds__(MAXW * 32, MINB) eri_kernel(const EriArgs a) {
                 }
             rp.s = __shfl_sync(0xffffffffu, rp.s, 0);
             rp.ph = __shfl_sync(0xffffffffu, rp.ph, 0);
+        } else if (NBW > 1 && helper) {
+            if (nhave) build_r(nquartet, nkq, nkp, [] {});
         } else if (!active) {
             // a warp without rows still takes part in the ring protocol
             for (int jq = last_kp ? 0 : a.ncb_q; jq < a.ncb_q; ++jq) {
@@ -558,7 +573,7 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
     const long long nwork = a.qmajor ? a.nquartets : a.nquartets * a.ncta_per_q;
     const long long slots = (long long)ctx->num_sms * MINB;
     long long grid = nwork < slots ? nwork : slots;
-    kern<<<(unsigned)grid, (a.wpc + 1) * 32, lay.total, st>>>(a);
+    kern<<<(unsigned)grid, (a.wpc + builder_warps(MAXW)) * 32, lay.total, st>>>(a);
     ctx->launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) { ctx->err = std::string("eri_kernel launch: ") + cudaGetErrorString(e); return MD4_ECUDA; }
@@ -567,7 +582,8 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
 
 template <int NT_CD, bool EXACT>
 md4_status launch_w(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
-    if (a.wpc + 1 <= 9) return launch_one<NT_CD, 8, 9, EXACT, 1>(ctx, a, st);
+    if (a.wpc <= 7) return launch_one<NT_CD, 8, 9, EXACT, 1>(ctx, a, st);
+    if (a.wpc == 8) return launch_one<NT_CD, 8, 10, EXACT, 1>(ctx, a, st);
     return launch_one<NT_CD, 8, 12, EXACT, 1>(ctx, a, st);
 }
 
