@@ -99,12 +99,18 @@ md4_status md4_set_kernel(md4_ctx* ctx, int kind, double omega);
  * npair == 0 gives a valid empty list.  *out is NULL on failure.  The call validates, copies ij and
  * enqueues the pair kernel on the context's internal stream; it does not wait for the kernel (it blocks only
  * when it is several builds ahead of the device).  Device memory comes from the context's pool of released
- * lists when a block of about that size is there (at most 4 GB are kept idle; env MD4_POOL_MAX_MB). */
+ * lists when a block of about that size is there (at most max(4 GB, 1/8 of the device memory) are kept idle -- a batch
+ * loop that frees a step's lists before building the next step's gets them all back without cudaMalloc; env
+ * MD4_POOL_MAX_MB overrides; md4_trim returns the idle blocks to the driver). */
 md4_status md4_build_pairs(md4_ctx* ctx, int npair, const int* ij, md4_pairs** out);
 
 /* Release one pair list (also done by md4_destroy).  NULL is a no-op.  Does not synchronise: launches that still
  * read the list finish first, on the device, before its memory is overwritten by a later md4_build_pairs. */
 void md4_free_pairs(md4_ctx* ctx, md4_pairs* pairs);
+
+/* Return every idle block of the context's pool to the driver (cudaFree; waits for the launches that still read them).
+ * For callers whose own allocator runs short of device memory; the pool refills as lists are released. */
+md4_status md4_trim(md4_ctx* ctx);
 
 /* Make cuda_stream wait, on the device, until the pair kernel of `pairs` has finished (the call itself returns at
  * once).  md4_compute does this for both of its lists; the call is for a caller that orders its own work -- or its

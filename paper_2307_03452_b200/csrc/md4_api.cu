@@ -1,6 +1,7 @@
 // md4_api.cu -- the C ABI of include/md4.h: context, shells, pair lists, compute dispatch.
 // Host logic only; every step of the hot path runs in the kernels of md4_pairs.cu / md4_eri.cu.
 #include <cmath>
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -48,7 +49,7 @@ void free_shells(md4_ctx* c, bool release = false) {
 // A released list's block goes here together with the event of its last reader; the next md4_build_pairs of about
 // that size takes it and makes its pair kernel wait for that event on the device.  Nothing here blocks the host.
 constexpr size_t POOL_MIN_BYTES = (size_t)64 << 10;          // smaller blocks go straight to cudaMalloc/cudaFree
-constexpr size_t POOL_MAX_DEFAULT = (size_t)4 << 30;         // bytes kept idle at most (env MD4_POOL_MAX_MB overrides)
+constexpr size_t POOL_MAX_FLOOR = (size_t)4 << 30;           // bytes kept idle at most: max(this, 1/8 of the device memory); env MD4_POOL_MAX_MB overrides
 
 void pool_release(md4_ctx* c) {
     for (auto& kv : c->pool) {
@@ -180,7 +181,9 @@ md4_status md4_create(md4_ctx** out, int cuda_device) {
     }
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->build_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->tacc_free, cudaEventDisableTiming);
-    c->pool_max_bytes = POOL_MAX_DEFAULT;
+    // a batch loop frees all lists of a step before it builds the next step's: the idle pool must hold a step's working set
+    // (13 GB for the 42 batches of cfg5), or every big list goes through cudaFree + cudaMalloc, each a device-wide sync
+    c->pool_max_bytes = std::max(POOL_MAX_FLOOR, (size_t)prop.totalGlobalMem / 8);
     if (const char* env = std::getenv("MD4_POOL_MAX_MB")) {
         const long long mb = std::atoll(env);
         if (mb >= 0) c->pool_max_bytes = (size_t)mb << 20;
@@ -496,6 +499,13 @@ md4_status md4_compute(md4_ctx* ctx, const md4_pairs* bra, const md4_pairs* ket,
     if (s != MD4_OK) return s;
     e = order_after(ctx, bra, ket, st);
     if (e != cudaSuccess) return cuda_fail(ctx, "md4_compute", e);
+    return MD4_OK;
+}
+
+md4_status md4_trim(md4_ctx* ctx) {
+    if (!ctx) return MD4_EINVAL;
+    DeviceGuard g(ctx->device);
+    pool_release(ctx);
     return MD4_OK;
 }
 

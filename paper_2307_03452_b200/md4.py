@@ -22,7 +22,7 @@ STATUS_NAMES = ["MD4_OK", "MD4_EINVAL", "MD4_EUNSUPPORTED", "MD4_ESTATE", "MD4_E
 SYMBOLS = [
     "md4_create", "md4_destroy", "md4_last_error", "md4_set_shells", "md4_build_pairs", "md4_free_pairs",
     "md4_stream_wait_pairs", "md4_set_kernel", "md4_num_ao", "md4_compute_jk", "md4_compute_jk_host",
-    "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host", "md4_compute_static",
+    "md4_pairs_count", "md4_pairs_class", "md4_output_size", "md4_compute", "md4_compute_host", "md4_compute_static", "md4_trim",
     "md4_launch_count", "md4_flops_per_quartet", "md4_debug_boys", "md4_debug_solid_coeff",
     "md4_debug_hermite_r", "md4_debug_pair_h", "md4_debug_work_items",
 ]
@@ -73,6 +73,8 @@ def load():
     lib.md4_compute_host.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, vp]
     lib.md4_compute_static.argtypes = [vp, vp, vp, vp, ctypes.c_size_t, vp]
     lib.md4_compute_static.restype = ctypes.c_int
+    lib.md4_trim.argtypes = [vp]
+    lib.md4_trim.restype = ctypes.c_int
     lib.md4_compute_host.restype = ctypes.c_int
     lib.md4_num_ao.argtypes = [vp, ip]
     lib.md4_num_ao.restype = ctypes.c_int
@@ -216,6 +218,10 @@ class Engine:
         self._check(load().md4_compute(self.handle, bra.handle, ket.handle, ctypes.c_void_p(out.data_ptr()),
                                        out.numel(), ctypes.c_void_p(stream)))
         return out.view(-1)[:n].view(self.output_shape(bra, ket)) if n else out.view(-1)[:0]
+
+    def trim(self):
+        """Return the idle blocks of the context's pool to the driver (md4_trim)."""
+        self._check(load().md4_trim(self.handle))
 
     def compute_static(self, bra: PairList, ket: PairList, out, stream=None):
         """Enqueue md4_compute_static (no device allocation: the [ab|q~] scratch of contracted bras is the library's static

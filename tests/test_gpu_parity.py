@@ -422,6 +422,33 @@ def test_free_and_rebuild_without_host_sync(eng):
         (outs[1].permute(1, 0, 4, 5, 2, 3) - ref).abs().max() <= 1e-12 * ref.abs().max()
 
 
+def test_trim_returns_the_idle_pool_and_lists_rebuild(eng):
+    """Released lists stay in the context's pool (no cudaFree); md4_trim gives the idle blocks back to the driver -- the
+    free device memory grows by the H blocks of the two lists -- and the next build / compute is unaffected."""
+    import torch
+
+    wl = inputs.config2()
+    s = wl.shells
+    eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
+    eng.trim()
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    ref = eng.compute(bra, ket).clone()
+    torch.cuda.synchronize()
+    held = torch.cuda.mem_get_info(0)[0]
+    bra.free(); ket.free()
+    assert torch.cuda.mem_get_info(0)[0] == held
+    eng.trim()
+    torch.cuda.synchronize()
+    # 2 lists x 64 (hh) pairs x 2 role copies of H, each 37 column blocks x 16 row blocks x 512 bytes
+    h_bytes = 2 * 64 * 2 * 37 * 16 * 512
+    assert torch.cuda.mem_get_info(0)[0] - held >= 0.9 * h_bytes
+    bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
+    out = eng.compute(bra, ket)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    bra.free(); ket.free()
+
+
 @pytest.mark.parametrize("which", ["cfg4", "cfg5 (ii|hh) K=3", "cfg5 (ii|ii) K=3", "cfg3"])
 def test_repeated_launches_are_bit_identical(eng, which):
     """Every quartet is computed by one CTA in a fixed summation order, so two launches of the same batch must agree bit
