@@ -449,17 +449,20 @@ def test_trim_returns_the_idle_pool_and_lists_rebuild(eng):
     bra.free(); ket.free()
 
 
-@pytest.mark.parametrize("which", ["cfg4", "cfg5 (ii|hh) K=3", "cfg5 (ii|ii) K=3", "cfg3"])
+@pytest.mark.parametrize("which", ["cfg4", "cfg5 (ii|hh) K=3", "cfg5 (ii|ii) K=3", "cfg3", "cfg2", "cfg5 (hh|gg) K=3", "cfg5 (ig|hg) K=1"])
 def test_repeated_launches_are_bit_identical(eng, which):
     """Every quartet is computed by one CTA in a fixed summation order, so two launches of the same batch must agree bit
     for bit on EVERY element.  This is the test that exposed a write-after-read race on the H_cd ring in round 2 (the
     assembler had moved the release of a ring stage ahead of the tensor instructions that wait for the stage's last
     loads; contracted classes with spilled accumulators then read refilled data now and then: errors of 1e-9 ... O(1) in
-    a few dozen of 1024 quartets, which the sampled oracle comparisons never hit).  Full launches, all elements."""
+    a few dozen of 1024 quartets, which the sampled oracle comparisons never hit).  Full launches, all elements.
+    cfg2, (hh|gg) and (ig|hg) run the instantiation in which four warps share the in-place R recurrence (a race between
+    them would show here first)."""
     import torch
 
     wl = {"cfg4": inputs.config4, "cfg3": inputs.config3, "cfg5 (ii|hh) K=3": lambda: inputs.config5(17, K=3),
-          "cfg5 (ii|ii) K=3": lambda: inputs.config5(20, K=3)}[which]()
+          "cfg5 (ii|ii) K=3": lambda: inputs.config5(20, K=3), "cfg2": inputs.config2,
+          "cfg5 (hh|gg) K=3": lambda: inputs.config5(3, K=3), "cfg5 (ig|hg) K=1": lambda: inputs.config5(7, K=1)}[which]()
     s = wl.shells
     eng.set_shells(s.centers, s.l, s.prim_offset, s.exponents, s.coefficients)
     bra, ket = eng.build_pairs(wl.bra_ij), eng.build_pairs(wl.ket_ij)
