@@ -204,7 +204,9 @@ double md4_flops_per_quartet(const md4_pairs* bra, const md4_pairs* ket);
 /* How md4_compute splits the (2li+1)(2lj+1) rows of a bra class into work items of 8-row blocks, one consumer warp
  * per block (host logic only, no device needed): out7 HOST [7] = number of items per quartet (1 to 3), first row
  * block of item 0..2, row blocks of item 0..2.  The FP64 tensor pipe of sm_100a is per SM sub-partition, so an item
- * of n blocks costs ceil(n/4) block-times; the split minimises their sum. */
+ * of n blocks costs ceil(n/4) block-times; the split minimises their sum.  (One exception is not reported here: under a
+ * ket of at most 16 eight-column blocks -- gg, hg, hh, ig -- a bra of 12 to 15 row blocks runs as ONE item of 12-15
+ * consumer warps at 128 registers.) */
 md4_status md4_debug_work_items(int li, int lj, int* out7);
 
 /* Boys function F_m(T), m = 0..mmax (mmax <= 4*MD4_LMAX), evaluated on the device by the same device

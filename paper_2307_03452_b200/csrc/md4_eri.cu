@@ -33,8 +33,9 @@ constexpr int MAX_STAGES = 16;
 
 // Kernel instantiations by MAXW: 12 = bras with 10-11 row blocks per item (gg, ih, ii: three consumer warps per
 // sub-partition) + 1 producer warp; 10 = bras with 8 row blocks per item (hh, ig: two consumer warps per sub-partition) + 4
-// warps that build R, one per sub-partition; 9 = bras with up to 7 (hg: 7 + 6) + 1 producer warp, which then sits on the
-// sub-partition with one consumer warp; 8 / 4 = small classes, 2 / 3 CTAs per SM.  Registers are allocated per 4 warps, so
+// warps that build R, one per sub-partition; 9 = bras with up to 7 (hg: 7 + 6 under ih / ii kets) + 1 producer warp, which
+// then sits on the sub-partition with one consumer warp; 16 = bras of 12-15 row blocks (hg, ig) as ONE item under kets of
+// at most 16 column blocks, 128 registers (see launch_eri_with); 8 / 4 = small classes, 2 / 3 CTAs per SM.  Registers are allocated per 4 warps, so
 // the 12 warps of MAXW = 10 cost no more than 9 (168 registers either way).
 // Why 4 builders: one producer warp took 6 % from the two consumer warps it shared a sub-partition with, and the other six
 // waited for those two at the block barrier; spread over the four sub-partitions the same work costs every warp 1.5 %
@@ -582,6 +583,9 @@ md4_status launch_one(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
 
 template <int NT_CD, bool EXACT>
 md4_status launch_w(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
+    if constexpr (NT_CD == 11 || NT_CD == 13 || NT_CD == 15 || NT_CD == 16) {
+        if (a.wpc > 11) return launch_one<NT_CD, 8, 16, EXACT, 1>(ctx, a, st);
+    }
     if (a.wpc <= 7) return launch_one<NT_CD, 8, 9, EXACT, 1>(ctx, a, st);
     if (a.wpc == 8) return launch_one<NT_CD, 8, 10, EXACT, 1>(ctx, a, st);
     return launch_one<NT_CD, 8, 12, EXACT, 1>(ctx, a, st);
@@ -628,6 +632,16 @@ static md4_status launch_eri_with(md4_ctx* ctx, const PairListDev& bra, const Pa
         return MD4_EUNSUPPORTED;
     }
     plan_items(a);
+    // Kets of at most 16 column blocks (gg, hg, hh, ig) need 44-64 accumulator registers: the kernel then runs at 128
+    // registers (with 0.2-3 kB of spills) and a CTA can hold 16 warps.  Bras of 12-15 row blocks (hg: 13, ig: 15) become ONE
+    // item with a consumer warp per row block (instantiation MAXW = 16): the same number of block-times (13: 2 + 2 -> 4,
+    // 15: 2 + 2 -> 4) but 3-4 warps per sub-partition instead of 2 to hide the gather latency, and R is built once per
+    // quartet instead of once per item.  (hg|hg) 53.7 -> 60.1 %, (ig|hg) 62.8 -> 72.4 %, (ig|ig) 65.4 -> 71.3 % of peak.
+    // 20 warps at 96 registers for hh bras (16 row blocks) were measured too: 52-56 % against 64-67 %.
+    if ((a.nrb_cd == 11 || a.nrb_cd == 13 || a.nrb_cd == 15 || a.nrb_cd == 16) && a.nrb_ab >= 12 && a.nrb_ab <= 15) {
+        a.ncta_per_q = 1; a.wpc = a.nrb_ab;
+        a.row0[0] = 0; a.nrows[0] = a.nrb_ab; a.row0[1] = a.row0[2] = 0; a.nrows[1] = a.nrows[2] = 0;
+    }
     a.nquartets = (long long)a.nbra * a.nket;
     a.qmajor = (a.ncta_per_q >= 2 && a.nrows[0] != a.nrows[a.ncta_per_q - 1]) ? 1 : 0;
     // strip height: the H matrices of a strip's bra pairs (K_bra matrices each) should stay L2-resident next to the kets

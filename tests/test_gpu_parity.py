@@ -568,7 +568,7 @@ def _jk_check(eng, wl, seed, both=True):
 
 @pytest.mark.parametrize("lclass,kclass", [((0, 0, 0, 0), (1, 1, 1, 1)), ((2, 1, 1, 2), (1, 2, 1, 1)), ((4, 4, 4, 4), (1, 1, 1, 1)),
                                            ((5, 4, 6, 4), (1, 1, 1, 1)), ((6, 5, 4, 4), (1, 1, 1, 1)), ((6, 6, 6, 6), (1, 1, 1, 1)),
-                                           ((6, 6, 6, 5), (2, 1, 1, 2))])
+                                           ((6, 6, 6, 5), (2, 1, 1, 2)), ((6, 4, 5, 4), (1, 2, 1, 1))])
 def test_digest_jk_small_classes(eng, lclass, kclass):
     """md4_compute_jk against the oracle leg (binary128 integrals, long-double contraction) on ragged 5 x 4 batches:
     every element of J and K."""
