@@ -48,6 +48,7 @@ __host__ __device__ constexpr int cta_warps_max(int maxw) { return maxw == 10 ? 
 // every slot; every extra k-block costs 4 registers and 4 moves per k-block, and the differences are 0-9 % (e.g. (ih|ih)
 // 7.91 / 8.17 / 8.02 / 8.17 ms, (hh|hh) with four builders 4.70 / 5.03 / 4.62 / - ms).
 __host__ __device__ constexpr int pf_depth(int maxw, int nt) {
+    if (maxw == 16) return 2;   // wide items at 128 registers: 1 / 2 / 3 / 5 measured, (ig|ig) 4.11 / 4.04 / 4.10 / 4.17 ms
     if (maxw == 10) return nt == 11 ? 1 : ((nt == 13 || nt == 15 || nt == 16) ? 4 : 2);
     if (maxw <= 9) return (nt == 11 || nt == 13) ? 4 : 2;
     return (nt == 15 || nt == 16) ? 5 : (nt == 18 ? 1 : 2);
