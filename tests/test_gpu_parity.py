@@ -613,7 +613,9 @@ def test_digest_jk_equals_contraction_of_stored_integrals(eng):
 
 # ------------------------------------------------------------------------ l = 7 shells (S:8(f) item 4)
 K_CLASSES = [((7, 0, 0, 0), (1, 1, 1, 1)), ((7, 7, 2, 2), (1, 1, 1, 1)), ((7, 4, 4, 4), (1, 2, 1, 1)), ((7, 7, 5, 5), (1, 1, 1, 1)),
-             ((6, 6, 7, 3), (1, 1, 1, 1)), ((4, 4, 7, 5), (1, 1, 1, 1)), ((7, 6, 6, 5), (1, 1, 1, 1)), ((3, 7, 7, 1), (2, 1, 1, 1))]
+             ((6, 6, 7, 3), (1, 1, 1, 1)), ((4, 4, 7, 5), (1, 1, 1, 1)), ((7, 6, 6, 5), (1, 1, 1, 1)), ((3, 7, 7, 1), (2, 1, 1, 1)),
+             # (kf| bras: 105 rows = 14 row blocks, one wide item of 14 consumer warps under gg / hh kets
+             ((7, 3, 4, 4), (1, 1, 1, 1)), ((7, 3, 5, 5), (1, 2, 1, 1))]
 
 
 @pytest.mark.parametrize("lclass,kclass", K_CLASSES)
