@@ -33,15 +33,17 @@ constexpr int MAX_STAGES = 16;
 
 // Kernel instantiations by MAXW: 12 = bras with 10-11 row blocks per item (gg, ih, ii: three consumer warps per
 // sub-partition) + 1 producer warp; 10 = bras with 8 row blocks per item (hh, ig: two consumer warps per sub-partition) + 4
-// warps that build R, one per sub-partition; 9 = bras with up to 7 (hg: 7 + 6 under ih / ii kets) + 1 producer warp, which
+// warps that build R, one per sub-partition; 11 = bras with 10 row blocks per item (ih: 10 + 8) under kets of at most 16
+// column blocks + 2 builder warps, which sit on the two sub-partitions with two consumer warps ((ih|hg) 64.7 -> 67.7 %,
+// (ih|ig) 68.3 -> 70.1 %; under ih kets one producer is as good: 73.5 %); 9 = bras with up to 7 (hg: 7 + 6 under ih / ii kets) + 1 producer warp, which
 // then sits on the sub-partition with one consumer warp; 16 = bras of 12-15 row blocks (hg, ig) as ONE item under kets of
 // at most 16 column blocks, 128 registers (see launch_eri_with); 8 / 4 = small classes, 2 / 3 CTAs per SM.  Registers are allocated per 4 warps, so
 // the 12 warps of MAXW = 10 cost no more than 9 (168 registers either way).
 // Why 4 builders: one producer warp took 6 % from the two consumer warps it shared a sub-partition with, and the other six
 // waited for those two at the block barrier; spread over the four sub-partitions the same work costs every warp 1.5 %
 // ((hh|gg) 2.90 -> 2.52 ms, (hh|hg) 3.80 -> 3.48, (ig|ig) 4.75 -> 4.53).
-__host__ __device__ constexpr int builder_warps(int maxw) { return maxw == 10 ? 4 : 1; }
-__host__ __device__ constexpr int cta_warps_max(int maxw) { return maxw == 10 ? 12 : maxw; }
+__host__ __device__ constexpr int builder_warps(int maxw) { return maxw == 10 ? 4 : (maxw == 11 ? 2 : 1); }
+__host__ __device__ constexpr int cta_warps_max(int maxw) { return (maxw == 10 || maxw == 11) ? 12 : maxw; }
 
 // How many k-blocks ahead GEMM1 loads its H_ab fragments (16 bytes per lane and k-block, from L2), per kernel
 // instantiation; nt = 8-column blocks of the ket.  Measured on the 21 classes of cfg5 (K = 1) with depths 1, 2, 4, 5 in
@@ -589,6 +591,9 @@ md4_status launch_w(md4_ctx* ctx, EriArgs& a, cudaStream_t st) {
     }
     if (a.wpc <= 7) return launch_one<NT_CD, 8, 9, EXACT, 1>(ctx, a, st);
     if (a.wpc == 8) return launch_one<NT_CD, 8, 10, EXACT, 1>(ctx, a, st);
+    if constexpr (NT_CD == 11 || NT_CD == 13 || NT_CD == 15 || NT_CD == 16) {
+        if (a.wpc == 10) return launch_one<NT_CD, 8, 11, EXACT, 1>(ctx, a, st);
+    }
     return launch_one<NT_CD, 8, 12, EXACT, 1>(ctx, a, st);
 }
 
